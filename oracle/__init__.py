@@ -1,0 +1,165 @@
+"""oracle -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+ctypes front end of ``oracle/mosaic_oracle.c``: the plain CPU (integer / binary64) statement of
+MOSAIC's confidence-gated aggregator stage (Sec. 4.2, Alg. 1, and
+the attention definition BASELINE.json's north_star fixes).  Only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may
+import this package.  It imports nothing from ``paper_2606_03014_b200`` and the CUDA path imports
+nothing from here.
+
+All arrays are numpy.  bf16 tensors are passed as ``uint16`` bit patterns.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "mosaic_oracle.c"
+_LIB = _HERE / "libmosaic_oracle.so"
+# No -ffast-math, no -march: the arithmetic is the C source's, in source order.
+_CFLAGS = ["-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-fno-fast-math", "-ffp-contract=off"]
+
+_lib = None
+
+
+def build(force: bool = False) -> Path:
+    """Compile the C oracle with gcc (building the checker is not using it)."""
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = _LIB.with_suffix(f".{os.getpid()}.tmp")
+        subprocess.run(["gcc", *_CFLAGS, str(_SRC), "-o", str(tmp), "-lm"], check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(str(_LIB))
+        p = ctypes.c_void_p
+        lib.oracle_gate.argtypes = [p, p, ctypes.c_int64, ctypes.c_int32, ctypes.c_float,
+                                    ctypes.c_int32, p, p, p, p, p]
+        lib.oracle_gate.restype = None
+        lib.oracle_compact.argtypes = [p, p, ctypes.c_int64, p, p, p, p]
+        lib.oracle_compact.restype = ctypes.c_int64
+        lib.oracle_attn_rows.argtypes = [p, p, p, p, ctypes.c_int64, p, p, p, ctypes.c_int32,
+                                         ctypes.c_int32, ctypes.c_int32, ctypes.c_float, p, p, p]
+        lib.oracle_attn_rows.restype = ctypes.c_int
+        lib.oracle_attn_full.argtypes = [p, p, p, p, ctypes.c_int32, ctypes.c_int32,
+                                         ctypes.c_int32, ctypes.c_int32, ctypes.c_float, p, p]
+        lib.oracle_attn_full.restype = ctypes.c_int
+        lib.oracle_num_threads.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _c(a, dtype):
+    a = np.ascontiguousarray(a, dtype=dtype)
+    return a
+
+
+def num_threads() -> int:
+    """Threads the attention oracle's OpenMP loops use (OMP_NUM_THREADS or all cores)."""
+    return int(_load().oracle_num_threads())
+
+
+def gate(answers, tau, expert_conf=None, conf_mode: int = 0):
+    """Alg. 1 lines 2-4 for every question.
+
+    answers int32 [Q,E]; tau is rounded to fp32 (reading G-4); expert_conf fp32 [Q,E] for
+    conf_mode 1.  Returns dict(mode, count, agree, conf, bypass).
+    """
+    answers = _c(answers, np.int32)
+    Q, E = answers.shape
+    if conf_mode not in (0, 1):
+        raise ValueError("conf_mode")
+    w = None
+    if conf_mode == 1:
+        w = _c(expert_conf, np.float32)
+        assert w.shape == (Q, E)
+    out = dict(mode=np.empty(Q, np.int32), count=np.empty(Q, np.int32),
+               agree=np.empty(Q, np.float32), conf=np.empty(Q, np.float32),
+               bypass=np.empty(Q, np.uint8))
+    _load().oracle_gate(_ptr(answers), _ptr(w), Q, E, ctypes.c_float(np.float32(tau)),
+                        conf_mode, _ptr(out["mode"]), _ptr(out["count"]), _ptr(out["agree"]),
+                        _ptr(out["conf"]), _ptr(out["bypass"]))
+    return out
+
+
+def compact(bypass, ctx_len):
+    """Alg. 1 line 6 survivors as a ragged batch (BJ:north_star).
+
+    Returns dict(survivor_idx int32 [S], cu_seqlens int64 [S+1], n_survivors, total_tokens,
+    max_seqlen).
+    """
+    bypass = _c(bypass, np.uint8)
+    ctx_len = _c(ctx_len, np.int32)
+    Q = bypass.shape[0]
+    assert ctx_len.shape == (Q,)
+    idx = np.empty(max(Q, 1), np.int32)
+    cu = np.empty(Q + 1, np.int64)
+    tot = np.zeros(1, np.int64)
+    mx = np.zeros(1, np.int32)
+    S = int(_load().oracle_compact(_ptr(bypass), _ptr(ctx_len), Q, _ptr(idx), _ptr(cu),
+                                   _ptr(tot), _ptr(mx)))
+    return dict(survivor_idx=idx[:S].copy(), cu_seqlens=cu[:S + 1].copy(), n_survivors=S,
+                total_tokens=int(tot[0]), max_seqlen=int(mx[0]))
+
+
+def _check_qkv(q, k, v, cu_seqlens):
+    q = _c(q, np.uint16)
+    k = _c(k, np.uint16)
+    v = _c(v, np.uint16)
+    cu = _c(cu_seqlens, np.int64)
+    T, Hq, D = q.shape
+    Tk, Hkv, Dk = k.shape
+    assert v.shape == k.shape and Tk == T and Dk == D and Hq % Hkv == 0
+    assert cu[0] == 0 and cu[-1] == T and np.all(np.diff(cu) >= 0)
+    return q, k, v, cu, T, Hq, Hkv, D
+
+
+def attn_rows(q, k, v, cu_seqlens, row_seq, row_head, row_pos, softmax_scale):
+    """Selected output rows (sequence, q head, position) of the attention definition.
+
+    q uint16 [T,Hq,D], k/v uint16 [T,Hkv,D] (bf16 bits).  Returns (O float64 [n,D],
+    LSE float64 [n], psum float64 [n]) where psum is the sum of the row's softmax weights.
+    """
+    q, k, v, cu, T, Hq, Hkv, D = _check_qkv(q, k, v, cu_seqlens)
+    rs = _c(row_seq, np.int32)
+    rh = _c(row_head, np.int32)
+    rp = _c(row_pos, np.int64)
+    n = rs.shape[0]
+    assert rh.shape == (n,) and rp.shape == (n,)
+    if n:
+        L = np.diff(cu)[rs]
+        assert np.all((rp >= 0) & (rp < L)) and np.all((rh >= 0) & (rh < Hq))
+    O = np.empty((n, D), np.float64)
+    lse = np.empty(n, np.float64)
+    ps = np.empty(n, np.float64)
+    rc = _load().oracle_attn_rows(_ptr(q), _ptr(k), _ptr(v), _ptr(cu), n, _ptr(rs), _ptr(rh),
+                                  _ptr(rp), Hq, Hkv, D, ctypes.c_float(np.float32(softmax_scale)),
+                                  _ptr(O), _ptr(lse), _ptr(ps))
+    if rc:
+        raise MemoryError("oracle_attn_rows")
+    return O, lse, ps
+
+
+def attn_full(q, k, v, cu_seqlens, softmax_scale):
+    """Every row: returns (O float64 [T,Hq,D], LSE float64 [Hq,T])."""
+    q, k, v, cu, T, Hq, Hkv, D = _check_qkv(q, k, v, cu_seqlens)
+    O = np.empty((T, Hq, D), np.float64)
+    lse = np.empty((Hq, T), np.float64)
+    rc = _load().oracle_attn_full(_ptr(q), _ptr(k), _ptr(v), _ptr(cu), cu.shape[0] - 1, Hq, Hkv,
+                                  D, ctypes.c_float(np.float32(softmax_scale)), _ptr(O), _ptr(lse))
+    if rc:
+        raise MemoryError("oracle_attn_full")
+    return O, lse

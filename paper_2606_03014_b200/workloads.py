@@ -1,0 +1,187 @@
+"""Seeded synthetic workloads shaped like MOSAIC's (BASELINE.json configs[0..4] = C1..C5).
+
+This module only draws INPUTS.  It holds none of the method's arithmetic (no vote, no scan, no
+softmax) and is the one module the tests hand to both the CUDA path and the oracle.  The recipe
+is stated in DESIGN.md ("Input recipe"); the paper's own benchmarks (MMLU-Pro, MedMCQA, GPQA;
+PAPER.md P:L331-346) and expert traces are not available, these inputs stand in for them with
+their shapes: 10-option multiple-choice labels, k = 3..8 experts, instruction-length vs
+long-reasoning traces, 32k-class contexts.
+
+Every array comes from numpy.random.Generator(PCG64(SeedSequence([seed, config_id, array_id]))).
+Q/K/V come from a seeded torch generator on the device that will consume them (CPU for the small
+configs, CUDA for the large ones) -- a fixed bit pattern for a given (seed, config, device kind).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import Optional
+
+import numpy as np
+
+# array ids (third word of the seed sequence)
+_A_CONSENSUS, _A_AGREE, _A_OTHER, _A_WEIGHT, _A_CTX, _A_CTX2, _A_CTX3, _A_QKV = range(8)
+
+
+def rng(seed: int, config_id: int, array_id: int) -> np.random.Generator:
+    return np.random.Generator(np.random.PCG64(np.random.SeedSequence([seed, config_id, array_id])))
+
+
+@dataclass(frozen=True)
+class Config:
+    """One BASELINE.json config.  `name` is what bench.py prints in config.workload."""
+    config_id: int
+    name: str
+    Q: int                      # questions entering the gate
+    E: int                      # experts per question (the paper's k)
+    p_agree: float              # P(an expert gives the consensus answer)
+    tau: float                  # gate threshold (1 and 2/3 are the paper's points)
+    has_conf: bool              # fp32 expert confidences present (conf_mode 1 also run)
+    Hq: int
+    Hkv: int
+    D: int
+    ctx: str                    # context-length recipe, see ctx_len()
+    k_scale: float = 1.0        # C4 multiplies K by 2 to sharpen the softmax
+    max_attn_seqs: Optional[int] = None   # C5: attention over the first 16 survivors only
+    n_options: int = 10
+
+
+C1 = Config(1, "C1-tiny", 8, 3, 0.6, 2.0 / 3.0, False, 4, 2, 64, "uniform64_256")
+C2 = Config(2, "C2-instruction", 256, 3, 0.6, 2.0 / 3.0, True, 28, 4, 128, "prompt256+3xLN600")
+C3 = Config(3, "C3-reasoning-heavy", 64, 5, 0.6, 0.6, False, 28, 4, 128,
+            "prompt256+3xLN600+2xLN6000")
+C4 = Config(4, "C4-skewed", 512, 4, 0.6, 0.75, False, 32, 8, 128, "mix_1in8_long", k_scale=2.0)
+C5 = Config(5, "C5-large-sweep", 1 << 20, 8, 0.6, 0.75, True, 64, 8, 128, "uniform8k_32k",
+            max_attn_seqs=16)
+CONFIGS = {c.config_id: c for c in (C1, C2, C3, C4, C5)}
+C5_SWEEP = [(p, tau) for p in (0.3, 0.6, 0.9) for tau in (0.5, 0.75)]
+
+
+def answers(cfg: Config, seed: int, p_agree: Optional[float] = None, Q: Optional[int] = None):
+    """int32 [Q,E]: a consensus label g ~ U{0..9} per question; each expert independently
+    answers g with probability p, otherwise one of the other nine labels uniformly."""
+    Q = cfg.Q if Q is None else Q
+    p = cfg.p_agree if p_agree is None else p_agree
+    g = rng(seed, cfg.config_id, _A_CONSENSUS).integers(0, cfg.n_options, size=Q, dtype=np.int32)
+    hit = rng(seed, cfg.config_id, _A_AGREE).random((Q, cfg.E)) < p
+    other = rng(seed, cfg.config_id, _A_OTHER).integers(0, cfg.n_options - 1, size=(Q, cfg.E),
+                                                        dtype=np.int32)
+    other = other + (other >= g[:, None])
+    return np.where(hit, g[:, None], other).astype(np.int32)
+
+
+def expert_conf(cfg: Config, seed: int, Q: Optional[int] = None):
+    """fp32 [Q,E] ~ U[0,1) on the 2^-24 grid, so binary64 sums of a row are exact."""
+    Q = cfg.Q if Q is None else Q
+    u = rng(seed, cfg.config_id, _A_WEIGHT).integers(0, 1 << 32, size=(Q, cfg.E), dtype=np.uint64)
+    return ((u >> 8).astype(np.float64) * 2.0 ** -24).astype(np.float32)
+
+
+def _lognormal_len(g: np.random.Generator, median: float, sigma: float, cap: int, size):
+    x = np.rint(g.lognormal(np.log(median), sigma, size=size))
+    return np.minimum(cap, np.maximum(1, x)).astype(np.int64)
+
+
+def ctx_len(cfg: Config, seed: int, Q: Optional[int] = None):
+    """int32 [Q]: tokens in question q's aggregator context = prompt + all expert traces."""
+    Q = cfg.Q if Q is None else Q
+    g = rng(seed, cfg.config_id, _A_CTX)
+    if cfg.ctx == "uniform64_256":
+        n = g.integers(64, 257, size=Q)
+    elif cfg.ctx == "prompt256+3xLN600":
+        n = 256 + _lognormal_len(g, 600.0, 0.5, 4096, (Q, 3)).sum(axis=1)
+    elif cfg.ctx == "prompt256+3xLN600+2xLN6000":
+        g2 = rng(seed, cfg.config_id, _A_CTX2)
+        n = (256 + _lognormal_len(g, 600.0, 0.5, 4096, (Q, 3)).sum(axis=1)
+             + _lognormal_len(g2, 6000.0, 0.5, 16384, (Q, 2)).sum(axis=1))
+    elif cfg.ctx == "mix_1in8_long":
+        g2 = rng(seed, cfg.config_id, _A_CTX2)
+        g3 = rng(seed, cfg.config_id, _A_CTX3)
+        is_long = g.random(Q) < 0.125
+        n = np.where(is_long, g2.integers(4000, 10001, size=Q), g3.integers(300, 801, size=Q))
+    elif cfg.ctx == "uniform8k_32k":
+        n = g.integers(8192, 32769, size=Q)
+    else:
+        raise ValueError(cfg.ctx)
+    return n.astype(np.int32)
+
+
+@dataclass
+class GateInputs:
+    answers: np.ndarray
+    expert_conf: Optional[np.ndarray]
+    ctx_len: np.ndarray
+    tau: float
+    E: int
+    extra: dict = field(default_factory=dict)
+
+
+def gate_inputs(cfg: Config, seed: int, p_agree: Optional[float] = None,
+                tau: Optional[float] = None, Q: Optional[int] = None) -> GateInputs:
+    return GateInputs(answers(cfg, seed, p_agree, Q),
+                      expert_conf(cfg, seed, Q) if cfg.has_conf else None,
+                      ctx_len(cfg, seed, Q), cfg.tau if tau is None else tau, cfg.E)
+
+
+def softmax_scale(cfg: Config) -> float:
+    return 1.0 / float(np.sqrt(cfg.D))
+
+
+def qkv(cfg: Config, seed: int, total_tokens: int, device="cpu"):
+    """bf16 Q [T,Hq,D], K,V [T,Hkv,D] ~ N(0,1) (fp32 draws rounded to nearest-even), K times
+    cfg.k_scale.  torch is used for the bf16 dtype and, on CUDA, to draw in place in HBM."""
+    import torch
+
+    dev = torch.device(device)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(int(np.random.SeedSequence([seed, cfg.config_id, _A_QKV]).generate_state(1)[0]))
+
+    def draw(H, scale):
+        out = torch.empty((total_tokens, H, cfg.D), dtype=torch.bfloat16, device=dev)
+        step = max(1, (1 << 26) // (H * cfg.D))          # fp32 staging of <= 256 MiB
+        for t0 in range(0, total_tokens, step):
+            t1 = min(total_tokens, t0 + step)
+            x = torch.randn((t1 - t0, H, cfg.D), dtype=torch.float32, device=dev, generator=gen)
+            if scale != 1.0:
+                x = x * scale
+            out[t0:t1] = x.to(torch.bfloat16)
+        return out
+
+    return draw(cfg.Hq, 1.0), draw(cfg.Hkv, cfg.k_scale), draw(cfg.Hkv, 1.0)
+
+
+def sample_rows(cu_seqlens: np.ndarray, Hq: int, Hkv: int, seed: int, config_id: int,
+                n_random: int = 2048, tile: int = 128):
+    """Output rows (seq, head, pos) the O(L^2) oracle is asked for on the large configs:
+    tile-edge and sequence-edge rows of every sequence for one head per KV group, plus
+    n_random uniform draws half of which go to the shortest and the longest sequence."""
+    cu = np.asarray(cu_seqlens, np.int64)
+    L = np.diff(cu)
+    n_seqs = L.shape[0]
+    G = Hq // Hkv
+    g = rng(seed, config_id, 100)
+    rows = set()
+    for s in range(n_seqs):
+        if L[s] == 0:
+            continue
+        last_tile = tile * ((int(L[s]) - 1) // tile)
+        cand = {0, 1, tile - 1, tile, tile + 1, int(L[s]) - 2, int(L[s]) - 1, last_tile,
+                last_tile - 1, 2 * tile - 1, 2 * tile}
+        for i in cand:
+            if 0 <= i < L[s]:
+                for kvh in range(Hkv):
+                    h = kvh * G + int(g.integers(0, G))
+                    rows.add((s, h, int(i)))
+    nz = np.flatnonzero(L > 0)
+    if nz.size and n_random:
+        shortest, longest = nz[np.argmin(L[nz])], nz[np.argmax(L[nz])]
+        for r in range(n_random):
+            if r % 4 == 0:
+                s = int(shortest)
+            elif r % 4 == 1:
+                s = int(longest)
+            else:
+                s = int(nz[g.integers(0, nz.size)])
+            rows.add((s, int(g.integers(0, Hq)), int(g.integers(0, L[s]))))
+    rows = sorted(rows)
+    return (np.array([r[0] for r in rows], np.int32), np.array([r[1] for r in rows], np.int32),
+            np.array([r[2] for r in rows], np.int64))
