@@ -1,0 +1,193 @@
+/*
+ * mosaic.h -- C ABI of the confidence-gated aggregator stage of MOSAIC
+ * (arxiv/paper_2606_03014, "PAPER.md" cited as P:Lnn) for one NVIDIA B200 (sm_100a).
+ *
+ * The stage (Sec. 4.2 "adaptive aggregation"; Alg. 1):
+ *
+ *     for every question q with extracted expert answers a_1..a_k:
+ *         C(q) = max_a |{i : a_i = a}| / k                    (C_vote)
+ *         if C(q) >= tau:  y(q) = majority({a_i})             (aggregator skipped)
+ *         else:            y(q) = Aggregator(q, {a_i})        (the survivors)
+ *
+ * and the aggregator's prefill attention over each survivor's concatenated context (question
+ * prompt + all expert traces), which BASELINE.json's north_star fixes as variable-length
+ * causal grouped-query attention producing bf16 O and fp32 row logsumexp.
+ *
+ * Conventions (all entry points)
+ *   - Pointers marked [dev] are CUDA device pointers, 16-byte aligned, owned by the caller.
+ *     Pointers marked [host] are ordinary host pointers.  The library allocates no device
+ *     memory and keeps no state between calls; scratch comes from caller workspaces sized by
+ *     the *_workspace_bytes helpers.
+ *   - cuda_stream is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls
+ *     marked "async" only enqueue work on that stream and never synchronise.
+ *   - Errors are return codes; nothing is thrown or printed.  Host-visible arguments are
+ *     validated (MOSAIC_ERR_INVALID_ARG / MOSAIC_ERR_UNSUPPORTED / MOSAIC_ERR_WORKSPACE_TOO_SMALL);
+ *     device-side contents (monotone cu_seqlens, non-negative ctx_len) are trusted.
+ *     MOSAIC_ERR_CUDA reports a failed CUDA call (mosaic_last_cuda_error() gives its code).
+ *   - There is no CPU fallback: without a CUDA device every compute call returns MOSAIC_ERR_CUDA.
+ */
+#ifndef MOSAIC_H_
+#define MOSAIC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    MOSAIC_OK = 0,
+    MOSAIC_ERR_INVALID_ARG = 1,
+    MOSAIC_ERR_UNSUPPORTED = 2,
+    MOSAIC_ERR_WORKSPACE_TOO_SMALL = 3,
+    MOSAIC_ERR_CUDA = 4
+} mosaic_status_t;
+
+/* Confidence estimator C(q) used by the gate (the gate "is agnostic to the choice of
+ * confidence estimator"). */
+enum {
+    MOSAIC_CONF_VOTE = 0,     /* C_vote = plurality fraction, the paper's instantiation */
+    MOSAIC_CONF_WEIGHTED = 1  /* extension (reading G-10): weight share of the modal answer */
+};
+
+#define MOSAIC_MAX_EXPERTS 32
+
+/* ---------------------------------------------------------------------------------------------
+ * mosaic_gate -- Alg. 1 lines 2-4 for Q questions, async.
+ *
+ *   answers     [dev] int32 [Q, E] row-major (question-major): a_i = Extract(E_i(q)).
+ *                     Any int32 is a label; only equality matters.
+ *   expert_conf [dev] fp32 [Q, E] per-response weights w; required iff conf_mode == WEIGHTED,
+ *                     else may be NULL.
+ *   Q, E              0 <= Q < 2^31, 1 <= E <= MOSAIC_MAX_EXPERTS (the paper's k; k = 3 at P:L331).
+ *   tau               threshold, compared in fp32 (reading G-4); NaN -> INVALID_ARG.
+ *   mode_out    [dev] int32 [Q]  majority({a_i}); ties -> smallest label (reading G-2). May be NULL.
+ *   count_out   [dev] int32 [Q]  c* = max_a |{i: a_i = a}|.                        May be NULL.
+ *   agree_out   [dev] fp32  [Q]  C_vote = fl32(c*) / fl32(E), one IEEE division.    May be NULL.
+ *   conf_out    [dev] fp32  [Q]  the C(q) the gate compared: agree (VOTE) or
+ *                                fl32(sum_{i: a_i = mode} w_i / sum_i w_i) with binary64 sums in
+ *                                expert order, agree when sum_i w_i <= 0 (WEIGHTED).  May be NULL.
+ *   bypass_out  [dev] uint8 [Q]  1 iff C(q) >= tau (aggregator skipped, answer = mode). Required.
+ *
+ * Q == 0 is a successful no-op.
+ * ------------------------------------------------------------------------------------------- */
+mosaic_status_t mosaic_gate(const int32_t* answers, const float* expert_conf, int64_t Q, int32_t E,
+                            float tau, int32_t conf_mode, int32_t* mode_out, int32_t* count_out,
+                            float* agree_out, float* conf_out, uint8_t* bypass_out,
+                            void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * mosaic_compact -- Alg. 1 line 6: the questions that failed the gate become the
+ * aggregator's ragged batch (north_star: "stream-compacts the surviving queries into a ragged
+ * batch with cu_seqlens"), async.  Stable: ascending question index (reading G-11).
+ *
+ *   bypass       [dev] uint8 [Q]   from mosaic_gate (0 = survivor).
+ *   ctx_len      [dev] int32 [Q]   tokens in question q's aggregator context (prompt + all expert
+ *                                  traces, reading G-12), >= 0.
+ *   survivor_idx [dev] int32 [Q]   capacity Q; first S entries written.
+ *   cu_seqlens   [dev] int64 [Q+1] capacity Q+1; first S+1 entries written: cu[0] = 0,
+ *                                  cu[j+1] = cu[j] + ctx_len[survivor_idx[j]].
+ *   n_survivors  [dev] int32 [1]   S.
+ *   total_tokens [dev] int64 [1]   cu[S].
+ *   max_seqlen   [dev] int32 [1]   max_j ctx_len[survivor_idx[j]] (0 if S == 0).
+ *   workspace    [dev] >= mosaic_compact_workspace_bytes(Q) bytes, contents arbitrary.
+ *
+ * Q == 0 writes S = 0, cu[0] = 0, total_tokens = 0, max_seqlen = 0.
+ * ------------------------------------------------------------------------------------------- */
+size_t mosaic_compact_workspace_bytes(int64_t Q);
+mosaic_status_t mosaic_compact(const uint8_t* bypass, const int32_t* ctx_len, int64_t Q,
+                               int32_t* survivor_idx, int64_t* cu_seqlens, int32_t* n_survivors,
+                               int64_t* total_tokens, int32_t* max_seqlen, void* workspace,
+                               size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * mosaic_gate_compact -- mosaic_gate followed by mosaic_compact in ONE kernel launch (the
+ * bypass mask never makes a round trip through HBM before the scan), async.  Same arguments,
+ * same results bit for bit; bypass_out may be NULL here.  Workspace: mosaic_compact's.
+ * ------------------------------------------------------------------------------------------- */
+mosaic_status_t mosaic_gate_compact(const int32_t* answers, const float* expert_conf,
+                                    const int32_t* ctx_len, int64_t Q, int32_t E, float tau,
+                                    int32_t conf_mode, int32_t* mode_out, int32_t* count_out,
+                                    float* agree_out, float* conf_out, uint8_t* bypass_out,
+                                    int32_t* survivor_idx, int64_t* cu_seqlens,
+                                    int32_t* n_survivors, int64_t* total_tokens,
+                                    int32_t* max_seqlen, void* workspace, size_t workspace_bytes,
+                                    void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * mosaic_agg_prefill_attn -- the aggregator's prefill attention over the survivors' packed
+ * contexts (math fixed by north_star), async.  For sequence s with tokens
+ * t0 = cu_seqlens[s] .. t0 + L - 1, q head h, kv head g = h / (Hq / Hkv), row i:
+ *
+ *     x_j = softmax_scale * sum_d Q[t0+i,h,d] K[t0+j,g,d],   j = 0..i  (causal, sequence-local)
+ *     LSE = ln sum_j exp(x_j)                    O_d = sum_j exp(x_j - LSE) V[t0+j,g,d]
+ *
+ *   q            [dev] bf16 [T, Hq, D]   packed, D fastest, no padding between sequences.
+ *   k, v         [dev] bf16 [T, Hkv, D]
+ *   cu_seqlens   [dev] int64 [n_seqs+1]  cu[0] = 0, non-decreasing, cu[n_seqs] = total_tokens.
+ *   n_seqs, total_tokens, max_seqlen     HOST values; max_seqlen >= every sequence length.
+ *                                        0 <= total_tokens < 2^31.
+ *   Hq, Hkv, D                           Hq % Hkv == 0; D in {64, 128} (else UNSUPPORTED).
+ *   softmax_scale                        finite fp32 (the configs use 1/sqrt(D)).
+ *   o            [dev] bf16 [T, Hq, D]   fp32 accumulator rounded to nearest-even.
+ *   lse          [dev] fp32 [Hq, T]      natural log, of the scaled scores.
+ *   workspace    [dev] >= mosaic_agg_prefill_attn_workspace_bytes(...) bytes, contents arbitrary.
+ *
+ * n_seqs == 0 or total_tokens == 0 is a successful no-op; zero-length sequences contribute no rows.
+ * ------------------------------------------------------------------------------------------- */
+size_t mosaic_agg_prefill_attn_workspace_bytes(int32_t n_seqs, int64_t total_tokens, int32_t Hq,
+                                               int32_t Hkv, int32_t D);
+mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k, const void* v,
+                                        const int64_t* cu_seqlens, int32_t n_seqs,
+                                        int64_t total_tokens, int32_t max_seqlen, int32_t Hq,
+                                        int32_t Hkv, int32_t D, float softmax_scale, void* o,
+                                        float* lse, void* workspace, size_t workspace_bytes,
+                                        void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * mosaic_stage_host -- the whole stage from HOST buffers (the end-to-end call): copies the gate
+ * inputs to the device, runs mosaic_gate_compact, reads S / total_tokens / max_seqlen back,
+ * copies the survivors' packed Q/K/V to the device, runs mosaic_agg_prefill_attn and copies every
+ * result back.  SYNCHRONOUS: returns after the results are in the host buffers.
+ *
+ *   answers_h, expert_conf_h, ctx_len_h  [host] as mosaic_gate / mosaic_compact.
+ *   mode_h, conf_h, bypass_h             [host] [Q] outputs (mode_h, conf_h may be NULL).
+ *   survivor_idx_h [host] int32 [Q], cu_seqlens_h [host] int64 [Q+1] capacities as mosaic_compact.
+ *   n_survivors_h, total_tokens_h, max_seqlen_h [host] scalars.
+ *   max_attn_seqs   attention runs over the first min(S, max_attn_seqs) survivors (< 0: all S).
+ *   q_h, k_h, v_h   [host] bf16 packed [T_cap, H, D] holding AT LEAST the tokens of those
+ *                   survivors, laid out by the cu_seqlens this call will compute (the caller
+ *                   knows ctx_len, hence the layout, once it knows the mask; pass buffers built
+ *                   for a previous identical gate, or sized for the worst case).
+ *   T_cap           rows available in q_h/k_h/v_h and o_h, lse_h row stride ([Hq, T_cap]).
+ *   o_h, lse_h      [host] outputs; lse_h is [Hq, T_attn] contiguous with T_attn = tokens attended.
+ *   arena           [dev] scratch of arena_bytes >= mosaic_stage_host_arena_bytes(...).
+ *
+ * Returns MOSAIC_ERR_WORKSPACE_TOO_SMALL if the survivors' tokens exceed T_cap or the arena.
+ * ------------------------------------------------------------------------------------------- */
+size_t mosaic_stage_host_arena_bytes(int64_t Q, int32_t E, int64_t T_cap, int32_t Hq, int32_t Hkv,
+                                     int32_t D);
+mosaic_status_t mosaic_stage_host(const int32_t* answers_h, const float* expert_conf_h,
+                                  const int32_t* ctx_len_h, int64_t Q, int32_t E, float tau,
+                                  int32_t conf_mode, int32_t* mode_h, float* conf_h,
+                                  uint8_t* bypass_h, int32_t* survivor_idx_h,
+                                  int64_t* cu_seqlens_h, int32_t* n_survivors_h,
+                                  int64_t* total_tokens_h, int32_t* max_seqlen_h,
+                                  int32_t max_attn_seqs, const void* q_h, const void* k_h,
+                                  const void* v_h, int64_t T_cap, int32_t Hq, int32_t Hkv,
+                                  int32_t D, float softmax_scale, void* o_h, float* lse_h,
+                                  void* arena, size_t arena_bytes, void* cuda_stream);
+
+/* Diagnostics. */
+const char* mosaic_status_string(mosaic_status_t status);
+int mosaic_version(void);            /* major*10000 + minor*100 + patch */
+int mosaic_last_cuda_error(void);    /* cudaError_t of the last failed CUDA call on this thread */
+/* Kernel launches this library has enqueued from this process since load (every kernel counts 1;
+ * memsets and copies do not).  bench.py reports the delta over its timed region. */
+int64_t mosaic_kernel_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MOSAIC_H_ */

@@ -1,0 +1,150 @@
+// stage.cu -- mosaic_stage_host: the whole confidence-gated aggregator stage (Alg. 1)
+// from HOST buffers: H2D copies, gate + compaction, survivors' prefill attention, D2H copies.
+// Only marshalling lives here; every step of the path runs in the kernels of gate.cu / attn.cu.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "common.cuh"
+
+namespace mosaic {
+namespace {
+
+struct Arena {
+    int32_t* answers;
+    float* expert_conf;
+    int32_t* ctx_len;
+    int32_t* mode;
+    float* conf;
+    uint8_t* bypass;
+    int32_t* survivor_idx;
+    int64_t* cu_seqlens;
+    int32_t* n_survivors;   // 3 scalars share one 32-byte slot
+    int64_t* total_tokens;
+    int32_t* max_seqlen;
+    void* compact_ws;
+    size_t compact_ws_bytes;
+    void *q, *k, *v, *o;
+    float* lse;
+    void* attn_ws;
+    size_t attn_ws_bytes;
+    size_t total;
+};
+
+Arena carve_arena(void* base, int64_t Q, int32_t E, int64_t T_cap, int32_t Hq, int32_t Hkv,
+                  int32_t D) {
+    Arena a{};
+    char* p = static_cast<char*>(base);
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        char* r = p + off;
+        off += (bytes + 255) & ~size_t(255);
+        return r;
+    };
+    a.answers = reinterpret_cast<int32_t*>(take((size_t)Q * E * 4));
+    a.expert_conf = reinterpret_cast<float*>(take((size_t)Q * E * 4));
+    a.ctx_len = reinterpret_cast<int32_t*>(take((size_t)Q * 4));
+    a.mode = reinterpret_cast<int32_t*>(take((size_t)Q * 4));
+    a.conf = reinterpret_cast<float*>(take((size_t)Q * 4));
+    a.bypass = reinterpret_cast<uint8_t*>(take((size_t)Q));
+    a.survivor_idx = reinterpret_cast<int32_t*>(take((size_t)Q * 4));
+    a.cu_seqlens = reinterpret_cast<int64_t*>(take((size_t)(Q + 1) * 8));
+    char* sc = take(32);
+    a.total_tokens = reinterpret_cast<int64_t*>(sc);
+    a.n_survivors = reinterpret_cast<int32_t*>(sc + 8);
+    a.max_seqlen = reinterpret_cast<int32_t*>(sc + 12);
+    a.compact_ws_bytes = mosaic_compact_workspace_bytes(Q);
+    a.compact_ws = take(a.compact_ws_bytes);
+    a.q = take((size_t)T_cap * Hq * D * 2);
+    a.k = take((size_t)T_cap * Hkv * D * 2);
+    a.v = take((size_t)T_cap * Hkv * D * 2);
+    a.o = take((size_t)T_cap * Hq * D * 2);
+    a.lse = reinterpret_cast<float*>(take((size_t)T_cap * Hq * 4));
+    const int64_t max_seqs = Q < T_cap ? Q : T_cap;
+    a.attn_ws_bytes = mosaic_agg_prefill_attn_workspace_bytes((int32_t)max_seqs, T_cap, Hq, Hkv, D);
+    a.attn_ws = take(a.attn_ws_bytes);
+    a.total = off;
+    return a;
+}
+
+}  // namespace
+}  // namespace mosaic
+
+using namespace mosaic;
+
+extern "C" size_t mosaic_stage_host_arena_bytes(int64_t Q, int32_t E, int64_t T_cap, int32_t Hq,
+                                                int32_t Hkv, int32_t D) {
+    if (Q < 0 || E < 1 || T_cap < 0 || Hq < 1 || Hkv < 1 || D < 1) return 0;
+    return carve_arena(nullptr, Q, E, T_cap, Hq, Hkv, D).total;
+}
+
+extern "C" mosaic_status_t mosaic_stage_host(
+    const int32_t* answers_h, const float* expert_conf_h, const int32_t* ctx_len_h, int64_t Q,
+    int32_t E, float tau, int32_t conf_mode, int32_t* mode_h, float* conf_h, uint8_t* bypass_h,
+    int32_t* survivor_idx_h, int64_t* cu_seqlens_h, int32_t* n_survivors_h,
+    int64_t* total_tokens_h, int32_t* max_seqlen_h, int32_t max_attn_seqs, const void* q_h,
+    const void* k_h, const void* v_h, int64_t T_cap, int32_t Hq, int32_t Hkv, int32_t D,
+    float softmax_scale, void* o_h, float* lse_h, void* arena, size_t arena_bytes,
+    void* cuda_stream) {
+    if (Q < 0 || Q >= (1ll << 31) || E < 1 || E > MOSAIC_MAX_EXPERTS || T_cap < 0 || Hq < 1 ||
+        Hkv < 1 || Hq % Hkv != 0)
+        return MOSAIC_ERR_INVALID_ARG;
+    if (D != 64 && D != 128) return MOSAIC_ERR_UNSUPPORTED;
+    if (!bypass_h || !survivor_idx_h || !cu_seqlens_h || !n_survivors_h || !total_tokens_h ||
+        !max_seqlen_h || !arena || !aligned16(arena))
+        return MOSAIC_ERR_INVALID_ARG;
+    if (Q > 0 && (!answers_h || !ctx_len_h)) return MOSAIC_ERR_INVALID_ARG;
+    if (conf_mode == MOSAIC_CONF_WEIGHTED && Q > 0 && !expert_conf_h) return MOSAIC_ERR_INVALID_ARG;
+    Arena a = carve_arena(arena, Q, E, T_cap, Hq, Hkv, D);
+    if (arena_bytes < a.total) return MOSAIC_ERR_WORKSPACE_TOO_SMALL;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const cudaMemcpyKind H2D = cudaMemcpyHostToDevice, D2H = cudaMemcpyDeviceToHost;
+
+    if (Q > 0) {
+        MOSAIC_CUDA_TRY(cudaMemcpyAsync(a.answers, answers_h, (size_t)Q * E * 4, H2D, s));
+        if (conf_mode == MOSAIC_CONF_WEIGHTED)
+            MOSAIC_CUDA_TRY(cudaMemcpyAsync(a.expert_conf, expert_conf_h, (size_t)Q * E * 4, H2D, s));
+        MOSAIC_CUDA_TRY(cudaMemcpyAsync(a.ctx_len, ctx_len_h, (size_t)Q * 4, H2D, s));
+    }
+    mosaic_status_t st = mosaic_gate_compact(
+        a.answers, conf_mode == MOSAIC_CONF_WEIGHTED ? a.expert_conf : nullptr, a.ctx_len, Q, E, tau,
+        conf_mode, a.mode, nullptr, nullptr, a.conf, a.bypass, a.survivor_idx, a.cu_seqlens,
+        a.n_survivors, a.total_tokens, a.max_seqlen, a.compact_ws, a.compact_ws_bytes, s);
+    if (st != MOSAIC_OK) return st;
+
+    struct {
+        int64_t total;
+        int32_t S;
+        int32_t max_len;
+    } sc;
+    MOSAIC_CUDA_TRY(cudaMemcpyAsync(&sc, a.total_tokens, 16, D2H, s));
+    if (Q > 0) {
+        if (mode_h) MOSAIC_CUDA_TRY(cudaMemcpyAsync(mode_h, a.mode, (size_t)Q * 4, D2H, s));
+        if (conf_h) MOSAIC_CUDA_TRY(cudaMemcpyAsync(conf_h, a.conf, (size_t)Q * 4, D2H, s));
+        MOSAIC_CUDA_TRY(cudaMemcpyAsync(bypass_h, a.bypass, (size_t)Q, D2H, s));
+    }
+    MOSAIC_CUDA_TRY(cudaStreamSynchronize(s));
+    *n_survivors_h = sc.S;
+    *total_tokens_h = sc.total;
+    *max_seqlen_h = sc.max_len;
+    const int64_t S = sc.S;
+    if (S > 0) MOSAIC_CUDA_TRY(cudaMemcpyAsync(survivor_idx_h, a.survivor_idx, (size_t)S * 4, D2H, s));
+    MOSAIC_CUDA_TRY(cudaMemcpyAsync(cu_seqlens_h, a.cu_seqlens, (size_t)(S + 1) * 8, D2H, s));
+    MOSAIC_CUDA_TRY(cudaStreamSynchronize(s));
+
+    const int64_t n_att = (max_attn_seqs < 0 || max_attn_seqs > S) ? S : max_attn_seqs;
+    if (n_att == 0) return MOSAIC_OK;
+    const int64_t T = cu_seqlens_h[n_att];
+    if (T == 0) return MOSAIC_OK;
+    if (T > T_cap) return MOSAIC_ERR_WORKSPACE_TOO_SMALL;
+    if (!q_h || !k_h || !v_h || !o_h || !lse_h) return MOSAIC_ERR_INVALID_ARG;
+    MOSAIC_CUDA_TRY(cudaMemcpyAsync(a.q, q_h, (size_t)T * Hq * D * 2, H2D, s));
+    MOSAIC_CUDA_TRY(cudaMemcpyAsync(a.k, k_h, (size_t)T * Hkv * D * 2, H2D, s));
+    MOSAIC_CUDA_TRY(cudaMemcpyAsync(a.v, v_h, (size_t)T * Hkv * D * 2, H2D, s));
+    st = mosaic_agg_prefill_attn(a.q, a.k, a.v, a.cu_seqlens, (int32_t)n_att, T, sc.max_len, Hq,
+                                 Hkv, D, softmax_scale, a.o, a.lse, a.attn_ws, a.attn_ws_bytes, s);
+    if (st != MOSAIC_OK) return st;
+    MOSAIC_CUDA_TRY(cudaMemcpyAsync(o_h, a.o, (size_t)T * Hq * D * 2, D2H, s));
+    MOSAIC_CUDA_TRY(cudaMemcpyAsync(lse_h, a.lse, (size_t)T * Hq * 4, D2H, s));
+    MOSAIC_CUDA_TRY(cudaStreamSynchronize(s));
+    return MOSAIC_OK;
+}
