@@ -1,0 +1,247 @@
+"""ctypes binding over libmosaic.so (include/mosaic.h).  Argument marshalling only: every step of
+the path runs in the library's kernels.  torch is used for device memory and streams.
+
+There is no fallback: if the library is missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+from typing import Optional
+
+import torch
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libmosaic.so"
+
+OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE_TOO_SMALL, ERR_CUDA = range(5)
+CONF_VOTE, CONF_WEIGHTED = 0, 1
+
+_vp, _i32, _i64, _f32, _sz = (ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_float,
+                              ctypes.c_size_t)
+
+# name -> (restype, argtypes): every symbol include/mosaic.h declares
+SIGNATURES = {
+    "mosaic_gate": (ctypes.c_int, [_vp, _vp, _i64, _i32, _f32, _i32, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "mosaic_compact_workspace_bytes": (_sz, [_i64]),
+    "mosaic_compact": (ctypes.c_int, [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "mosaic_gate_compact": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _f32, _i32, _vp, _vp, _vp,
+                                           _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "mosaic_agg_prefill_attn_workspace_bytes": (_sz, [_i32, _i64, _i32, _i32, _i32]),
+    "mosaic_agg_prefill_attn": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i64, _i32, _i32, _i32,
+                                               _i32, _f32, _vp, _vp, _vp, _sz, _vp]),
+    "mosaic_stage_host_arena_bytes": (_sz, [_i64, _i32, _i64, _i32, _i32, _i32]),
+    "mosaic_stage_host": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _f32, _i32, _vp, _vp, _vp, _vp,
+                                         _vp, _vp, _vp, _vp, _i32, _vp, _vp, _vp, _i64, _i32, _i32,
+                                         _i32, _f32, _vp, _vp, _vp, _sz, _vp]),
+    "mosaic_status_string": (ctypes.c_char_p, [ctypes.c_int]),
+    "mosaic_version": (ctypes.c_int, []),
+    "mosaic_last_cuda_error": (ctypes.c_int, []),
+    "mosaic_kernel_launch_count": (_i64, []),
+}
+
+_lib = None
+
+
+class MosaicError(RuntimeError):
+    def __init__(self, call: str, status: int):
+        lib = load()
+        name = lib.mosaic_status_string(status).decode()
+        extra = f" (cudaError {lib.mosaic_last_cuda_error()})" if status == ERR_CUDA else ""
+        super().__init__(f"{call} failed: {name}{extra}")
+        self.status = status
+
+
+def load() -> ctypes.CDLL:
+    """Loads libmosaic.so; raises if it has not been built (python -m paper_2606_03014_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with "
+                               "`python -m paper_2606_03014_b200.build` (no CPU fallback exists)")
+        lib = ctypes.CDLL(str(LIB_PATH))
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def _check(call: str, status: int):
+    if status != OK:
+        raise MosaicError(call, status)
+
+
+def _dptr(t: Optional[torch.Tensor], dtype=None, name="tensor"):
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError(f"{name} must be a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"{name} must be {dtype}, got {t.dtype}")
+    return t.data_ptr()
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def version() -> int:
+    return load().mosaic_version()
+
+
+def kernel_launch_count() -> int:
+    return int(load().mosaic_kernel_launch_count())
+
+
+def gate(answers, tau, expert_conf=None, conf_mode=CONF_VOTE, *, want_count=True, want_agree=True,
+         out=None, stream=None):
+    """mosaic_gate.  answers int32 [Q,E] on the GPU.  Returns dict(mode,count,agree,conf,bypass)."""
+    Q, E = answers.shape
+    dev = answers.device
+    o = out or {}
+    mode = o.get("mode", torch.empty(Q, dtype=torch.int32, device=dev))
+    count = o.get("count", torch.empty(Q, dtype=torch.int32, device=dev) if want_count else None)
+    agree = o.get("agree", torch.empty(Q, dtype=torch.float32, device=dev) if want_agree else None)
+    conf = o.get("conf", torch.empty(Q, dtype=torch.float32, device=dev))
+    bypass = o.get("bypass", torch.empty(Q, dtype=torch.uint8, device=dev))
+    st = load().mosaic_gate(_dptr(answers, torch.int32, "answers"),
+                            _dptr(expert_conf, torch.float32, "expert_conf"), Q, E, float(tau),
+                            conf_mode, _dptr(mode), _dptr(count), _dptr(agree), _dptr(conf),
+                            _dptr(bypass), _stream(stream))
+    _check("mosaic_gate", st)
+    return dict(mode=mode, count=count, agree=agree, conf=conf, bypass=bypass)
+
+
+def compact_workspace_bytes(Q: int) -> int:
+    return int(load().mosaic_compact_workspace_bytes(Q))
+
+
+def _compact_outputs(Q, dev, out):
+    o = out or {}
+    return dict(
+        survivor_idx=o.get("survivor_idx", torch.empty(max(Q, 1), dtype=torch.int32, device=dev)),
+        cu_seqlens=o.get("cu_seqlens", torch.empty(Q + 1, dtype=torch.int64, device=dev)),
+        n_survivors=o.get("n_survivors", torch.empty(1, dtype=torch.int32, device=dev)),
+        total_tokens=o.get("total_tokens", torch.empty(1, dtype=torch.int64, device=dev)),
+        max_seqlen=o.get("max_seqlen", torch.empty(1, dtype=torch.int32, device=dev)),
+        workspace=o.get("workspace", torch.empty(compact_workspace_bytes(Q), dtype=torch.uint8,
+                                                 device=dev)))
+
+
+def compact(bypass, ctx_len, *, out=None, stream=None):
+    """mosaic_compact.  Returns device tensors (full-capacity survivor_idx / cu_seqlens plus the
+    three device scalars); nothing is copied to the host."""
+    Q = bypass.shape[0]
+    r = _compact_outputs(Q, bypass.device, out)
+    st = load().mosaic_compact(_dptr(bypass, torch.uint8, "bypass"),
+                               _dptr(ctx_len, torch.int32, "ctx_len"), Q,
+                               _dptr(r["survivor_idx"]), _dptr(r["cu_seqlens"]),
+                               _dptr(r["n_survivors"]), _dptr(r["total_tokens"]),
+                               _dptr(r["max_seqlen"]), _dptr(r["workspace"]),
+                               r["workspace"].numel(), _stream(stream))
+    _check("mosaic_compact", st)
+    return r
+
+
+def gate_compact(answers, ctx_len, tau, expert_conf=None, conf_mode=CONF_VOTE, *, want_count=False,
+                 want_agree=False, want_bypass=True, out=None, stream=None):
+    """mosaic_gate_compact: both steps in one launch."""
+    Q, E = answers.shape
+    dev = answers.device
+    o = out or {}
+    r = _compact_outputs(Q, dev, out)
+    r["mode"] = o.get("mode", torch.empty(Q, dtype=torch.int32, device=dev))
+    r["count"] = o.get("count", torch.empty(Q, dtype=torch.int32, device=dev) if want_count else None)
+    r["agree"] = o.get("agree", torch.empty(Q, dtype=torch.float32, device=dev) if want_agree else None)
+    r["conf"] = o.get("conf", torch.empty(Q, dtype=torch.float32, device=dev))
+    r["bypass"] = o.get("bypass", torch.empty(Q, dtype=torch.uint8, device=dev) if want_bypass else None)
+    st = load().mosaic_gate_compact(
+        _dptr(answers, torch.int32, "answers"), _dptr(expert_conf, torch.float32, "expert_conf"),
+        _dptr(ctx_len, torch.int32, "ctx_len"), Q, E, float(tau), conf_mode, _dptr(r["mode"]),
+        _dptr(r["count"]), _dptr(r["agree"]), _dptr(r["conf"]), _dptr(r["bypass"]),
+        _dptr(r["survivor_idx"]), _dptr(r["cu_seqlens"]), _dptr(r["n_survivors"]),
+        _dptr(r["total_tokens"]), _dptr(r["max_seqlen"]), _dptr(r["workspace"]),
+        r["workspace"].numel(), _stream(stream))
+    _check("mosaic_gate_compact", st)
+    return r
+
+
+def attn_workspace_bytes(n_seqs, total_tokens, Hq, Hkv, D) -> int:
+    return int(load().mosaic_agg_prefill_attn_workspace_bytes(n_seqs, total_tokens, Hq, Hkv, D))
+
+
+def agg_prefill_attn(q, k, v, cu_seqlens, n_seqs, max_seqlen, softmax_scale, *, o=None, lse=None,
+                     workspace=None, stream=None):
+    """mosaic_agg_prefill_attn.  q bf16 [T,Hq,D], k/v bf16 [T,Hkv,D], cu_seqlens int64 (device,
+    at least n_seqs+1 entries).  Returns (o bf16 [T,Hq,D], lse fp32 [Hq,T])."""
+    T, Hq, D = q.shape
+    Hkv = k.shape[1]
+    if k.shape != (T, Hkv, D) or v.shape != k.shape:
+        raise ValueError("k/v shape")
+    dev = q.device
+    if o is None:
+        o = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty((Hq, T), dtype=torch.float32, device=dev)
+    if workspace is None:
+        workspace = torch.empty(max(attn_workspace_bytes(n_seqs, T, Hq, Hkv, D), 16),
+                                dtype=torch.uint8, device=dev)
+    st = load().mosaic_agg_prefill_attn(
+        _dptr(q, torch.bfloat16, "q"), _dptr(k, torch.bfloat16, "k"), _dptr(v, torch.bfloat16, "v"),
+        _dptr(cu_seqlens, torch.int64, "cu_seqlens"), int(n_seqs), int(T), int(max_seqlen), Hq, Hkv,
+        D, float(softmax_scale), _dptr(o, torch.bfloat16, "o"), _dptr(lse, torch.float32, "lse"),
+        _dptr(workspace), workspace.numel(), _stream(stream))
+    _check("mosaic_agg_prefill_attn", st)
+    return o, lse
+
+
+def stage_host_arena_bytes(Q, E, T_cap, Hq, Hkv, D) -> int:
+    return int(load().mosaic_stage_host_arena_bytes(Q, E, T_cap, Hq, Hkv, D))
+
+
+def _hptr(t: Optional[torch.Tensor], name="tensor"):
+    if t is None:
+        return None
+    if t.is_cuda or not t.is_contiguous():
+        raise ValueError(f"{name} must be a contiguous host tensor")
+    return t.data_ptr()
+
+
+def stage_host(answers_h, expert_conf_h, ctx_len_h, tau, conf_mode, q_h, k_h, v_h, softmax_scale,
+               *, max_attn_seqs=-1, out_h=None, arena=None, stream=None):
+    """mosaic_stage_host: the whole stage from (ideally pinned) host tensors; synchronous.
+    out_h may carry preallocated pinned host outputs.  Returns the dict of host outputs."""
+    Q, E = answers_h.shape
+    T_cap, Hq, D = q_h.shape
+    Hkv = k_h.shape[1]
+    o = dict(out_h or {})
+
+    def host(name, shape, dtype):
+        if name not in o:
+            o[name] = torch.empty(shape, dtype=dtype)
+        return o[name]
+
+    host("mode", Q, torch.int32)
+    host("conf", Q, torch.float32)
+    host("bypass", Q, torch.uint8)
+    host("survivor_idx", max(Q, 1), torch.int32)
+    host("cu_seqlens", Q + 1, torch.int64)
+    host("n_survivors", 1, torch.int32)
+    host("total_tokens", 1, torch.int64)
+    host("max_seqlen", 1, torch.int32)
+    host("o", (T_cap, Hq, D), torch.bfloat16)
+    host("lse", Hq * T_cap, torch.float32)
+    if arena is None:
+        arena = torch.empty(stage_host_arena_bytes(Q, E, T_cap, Hq, Hkv, D), dtype=torch.uint8,
+                            device="cuda")
+    st = load().mosaic_stage_host(
+        _hptr(answers_h), _hptr(expert_conf_h), _hptr(ctx_len_h), Q, E, float(tau), conf_mode,
+        _hptr(o["mode"]), _hptr(o["conf"]), _hptr(o["bypass"]), _hptr(o["survivor_idx"]),
+        _hptr(o["cu_seqlens"]), _hptr(o["n_survivors"]), _hptr(o["total_tokens"]),
+        _hptr(o["max_seqlen"]), int(max_attn_seqs), _hptr(q_h), _hptr(k_h), _hptr(v_h), T_cap, Hq,
+        Hkv, D, float(softmax_scale), _hptr(o["o"]), _hptr(o["lse"]), _dptr(arena), arena.numel(),
+        _stream(stream))
+    _check("mosaic_stage_host", st)
+    return o

@@ -1,0 +1,177 @@
+"""GPU parity, step 2: mosaic_agg_prefill_attn against the fp64 oracle.  Tolerances are
+BASELINE.json's: max |dO| <= 2e-2, max |dLSE| <= 1e-3.  Small cases are compared in full; the
+large configs on sampled rows plus structured inputs whose exact answer costs O(T*D) on the CPU
+(identical keys -> causal prefix mean of V and LSE = scale*q.k + ln(i+1), which counts the
+unmasked keys of EVERY row)."""
+import numpy as np
+import pytest
+import torch
+
+import _parity as P
+import oracle
+from paper_2606_03014_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def _cu(lengths):
+    return np.concatenate([[0], np.cumsum(np.asarray(lengths, np.int64))]).astype(np.int64)
+
+
+def _full_case(lengths, Hq, Hkv, D, seed, scale=None, k_scale=1.0):
+    cu = _cu(lengths)
+    T = int(cu[-1])
+    q = P.randn_bf16((T, Hq, D), seed)
+    k = P.randn_bf16((T, Hkv, D), seed + 1, k_scale)
+    v = P.randn_bf16((T, Hkv, D), seed + 2)
+    scale = 1.0 / np.sqrt(D) if scale is None else scale
+    o, lse = P.run_attn(q, k, v, cu, scale)
+    return P.check_attn_full(o, lse, q, k, v, cu, scale)
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_c1_tiny_full(seed):
+    """BASELINE configs[0]: D = 64, 4 q / 2 kv heads, lengths 64-256, every row compared."""
+    cfg = wl.C1
+    gi = wl.gate_inputs(cfg, seed)
+    oc = oracle.compact(oracle.gate(gi.answers, gi.tau)["bypass"], gi.ctx_len)
+    cu = oc["cu_seqlens"]
+    if oc["n_survivors"] == 0:
+        pytest.skip("no survivors for this seed")
+    q, k, v = wl.qkv(cfg, seed, int(cu[-1]))
+    scale = wl.softmax_scale(cfg)
+    o, lse = P.run_attn(q, k, v, cu, scale)
+    eo, el = P.check_attn_full(o, lse, q, k, v, cu, scale)
+    assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
+
+
+@pytest.mark.parametrize("D,Hq,Hkv", [(128, 8, 2), (64, 4, 2), (128, 7, 1), (64, 3, 3)])
+def test_ragged_edges_full(D, Hq, Hkv):
+    """Lengths around every tile edge (1, 127, 128, 129, 255, 256, 257, ...), zero-length
+    sequences in between, several tiles and a ragged tail; every row compared."""
+    lengths = [1, 0, 127, 128, 129, 0, 255, 256, 257, 2, 385, 640, 777]
+    eo, el = _full_case(lengths, Hq, Hkv, D, seed=11)
+    assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
+
+
+def test_sharp_softmax_and_scales():
+    """K x 2 (configs[3]) and K x 8 drive the running-max rescale path; scale = 0 gives uniform
+    weights; a negative scale flips the order of the scores."""
+    for k_scale, scale in ((2.0, None), (8.0, None), (1.0, 0.0), (1.0, -0.11)):
+        eo, el = _full_case([300, 513, 64], 4, 2, 128, seed=5, scale=scale, k_scale=k_scale)
+        assert eo <= P.O_TOL and el <= P.LSE_TOL, (k_scale, scale, eo, el)
+
+
+def test_single_token_sequences_return_v():
+    """L = 1 -> O = V exactly and LSE = scale * q.k (north_star invariant)."""
+    n, Hq, Hkv, D = 37, 8, 4, 128
+    cu = _cu([1] * n)
+    q, k, v = P.randn_bf16((n, Hq, D), 1), P.randn_bf16((n, Hkv, D), 2), P.randn_bf16((n, Hkv, D), 3)
+    o, lse = P.run_attn(q, k, v, cu, 0.25)
+    want = v.repeat_interleave(Hq // Hkv, dim=1)
+    assert torch.equal(o.cpu(), want)
+    dots = 0.25 * (q.double() * k.repeat_interleave(Hq // Hkv, dim=1).double()).sum(-1)  # [n,Hq]
+    assert float((lse.cpu().double() - dots.T).abs().max()) <= P.LSE_TOL
+
+
+def _identical_keys_check(lengths, Hq, Hkv, D, seed):
+    """Every key of a (sequence, kv head) identical: O_i = mean_{j<=i} V_j, LSE_i = s*q_i.k + ln(i+1).
+    Exact expected values by cumulative sums in float64 -- full coverage at any size."""
+    cu = _cu(lengths)
+    T = int(cu[-1])
+    dev = "cuda"
+    g = torch.Generator(device=dev).manual_seed(seed)
+    q = torch.randn((T, Hq, D), generator=g, device=dev).to(torch.bfloat16)
+    v = torch.randn((T, Hkv, D), generator=g, device=dev).to(torch.bfloat16)
+    kseq = torch.randn((len(lengths), Hkv, D), generator=g, device=dev).to(torch.bfloat16)
+    seq_of = torch.repeat_interleave(torch.arange(len(lengths), device=dev),
+                                     torch.tensor(lengths, device=dev))
+    k = kseq[seq_of].contiguous()
+    scale = 1.0 / np.sqrt(D)
+    o, lse = P.run_attn(q, k, v, cu, scale)
+    pos = torch.arange(T, device=dev) - torch.from_numpy(cu[:-1]).to(dev)[seq_of]
+    G = Hq // Hkv
+    worst_o = worst_l = 0.0
+    for s0 in range(0, len(lengths)):
+        a, b = int(cu[s0]), int(cu[s0 + 1])
+        if a == b:
+            continue
+        vm = torch.cumsum(v[a:b].double(), 0) / (pos[a:b].double() + 1)[:, None, None]
+        want_o = vm.repeat_interleave(G, dim=1)
+        worst_o = max(worst_o, float((o[a:b].double() - want_o).abs().max()))
+        dots = scale * (q[a:b].double() * k[a:b].repeat_interleave(G, dim=1).double()).sum(-1)
+        want_l = dots + torch.log(pos[a:b].double() + 1)[:, None]
+        worst_l = max(worst_l, float((lse[:, a:b].double().T - want_l).abs().max()))
+    return worst_o, worst_l
+
+
+def test_identical_keys_prefix_mean_every_row():
+    eo, el = _identical_keys_check([1, 130, 4097, 513, 9000, 255], 8, 2, 128, seed=3)
+    assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
+    eo, el = _identical_keys_check([200, 64, 1000], 4, 2, 64, seed=4)
+    assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
+
+
+def _config_batch(cfg, seed):
+    gi = wl.gate_inputs(cfg, seed)
+    og = oracle.gate(gi.answers, gi.tau)
+    oc = oracle.compact(og["bypass"], gi.ctx_len)
+    n = oc["n_survivors"] if cfg.max_attn_seqs is None else min(cfg.max_attn_seqs, oc["n_survivors"])
+    return oc["cu_seqlens"][:n + 1]
+
+
+@pytest.mark.parametrize("cid,n_random", [(2, 1024), (3, 512), (4, 1024), (5, 256)])
+def test_configs_sampled_rows_and_structured(cid, n_random):
+    """BASELINE configs[1..4] at full size, in the launch configuration bench.py times: sampled
+    rows against the O(L^2) oracle (tile edges and sequence edges of every sequence, plus random
+    rows weighted to the shortest and longest), then the identical-keys check on every row."""
+    cfg = wl.CONFIGS[cid]
+    cu = _config_batch(cfg, 0)
+    T = int(cu[-1])
+    q, k, v = wl.qkv(cfg, 0, T, device="cuda")
+    scale = wl.softmax_scale(cfg)
+    o, lse = P.run_attn(q, k, v, cu, scale)
+    rs, rh, rp = wl.sample_rows(cu, cfg.Hq, cfg.Hkv, 0, cfg.config_id, n_random=n_random)
+    eo, el = P.check_attn_rows(o, lse, q, k, v, cu, rs, rh, rp, scale)
+    assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
+    del q, k, v, o, lse
+    torch.cuda.empty_cache()
+    eo, el = _identical_keys_check(np.diff(cu).tolist(), cfg.Hq, cfg.Hkv, cfg.D, seed=cid)
+    assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
+
+
+def test_empty_batches_are_noops():
+    from paper_2606_03014_b200 import mosaic
+    q = torch.zeros((0, 4, 64), dtype=torch.bfloat16, device="cuda")
+    k = torch.zeros((0, 2, 64), dtype=torch.bfloat16, device="cuda")
+    cu = torch.zeros(1, dtype=torch.int64, device="cuda")
+    o, lse = mosaic.agg_prefill_attn(q, k, k, cu, 0, 0, 0.125)
+    assert o.shape == (0, 4, 64) and lse.shape == (4, 0)
+    with pytest.raises(mosaic.MosaicError) as e:
+        mosaic.agg_prefill_attn(torch.zeros((8, 4, 96), dtype=torch.bfloat16, device="cuda"),
+                                torch.zeros((8, 2, 96), dtype=torch.bfloat16, device="cuda"),
+                                torch.zeros((8, 2, 96), dtype=torch.bfloat16, device="cuda"),
+                                torch.tensor([0, 8], device="cuda"), 1, 8, 0.1)
+    assert e.value.status == mosaic.ERR_UNSUPPORTED
+
+
+def test_stage_host_matches_oracle():
+    """The end-to-end host call (mosaic_stage_host) on configs[0]."""
+    from paper_2606_03014_b200 import mosaic
+    cfg = wl.C1
+    gi = wl.gate_inputs(cfg, 0)
+    want = P.oracle_gate_compact(gi, 0)
+    cu = want["cu_seqlens"]
+    T = int(cu[-1])
+    q, k, v = wl.qkv(cfg, 0, T)
+    scale = wl.softmax_scale(cfg)
+    r = mosaic.stage_host(torch.from_numpy(gi.answers), None, torch.from_numpy(gi.ctx_len), gi.tau,
+                          0, q, k, v, scale)
+    S = int(r["n_survivors"])
+    assert S == want["n_survivors"] and int(r["total_tokens"]) == T
+    assert np.array_equal(r["bypass"].numpy(), want["bypass"])
+    assert np.array_equal(r["survivor_idx"][:S].numpy(), want["survivor_idx"])
+    assert np.array_equal(r["cu_seqlens"][:S + 1].numpy(), cu)
+    O_ref, lse_ref = oracle.attn_full(P.bf16_bits(q), P.bf16_bits(k), P.bf16_bits(v), cu, scale)
+    assert np.abs(r["o"][:T].float().numpy() - O_ref).max() <= P.O_TOL
+    assert np.abs(r["lse"][:cfg.Hq * T].view(cfg.Hq, T).numpy() - lse_ref).max() <= P.LSE_TOL

@@ -1,0 +1,108 @@
+"""GPU parity, step 1: mosaic_gate / mosaic_compact / mosaic_gate_compact against the oracle,
+bit-exact (BASELINE.json north_star), on the five configs x seeds {0,1,2} (the paper's seed set,
+P:L350) plus the edge cases of the boundary."""
+import numpy as np
+import pytest
+import torch
+
+import _parity as P
+from paper_2606_03014_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+@pytest.mark.parametrize("cid", [1, 2, 3, 4])
+def test_configs_bit_exact(cid, seed):
+    from paper_2606_03014_b200 import mosaic  # noqa: F401  (fails loudly if the .so is missing)
+    cfg = wl.CONFIGS[cid]
+    gi = wl.gate_inputs(cfg, seed)
+    for conf_mode in ([0, 1] if cfg.has_conf else [0]):
+        want = P.oracle_gate_compact(gi, conf_mode)
+        sep, fused = P.gpu_gate_compact_all(gi, conf_mode)
+        P.assert_gate_equal(sep, want)
+        P.assert_gate_equal(fused, want)
+
+
+@pytest.mark.parametrize("p_agree,tau", wl.C5_SWEEP)
+def test_c5_sweep_bit_exact(p_agree, tau):
+    """2^20 questions, E = 8, both confidence modes, int64 cu_seqlens past 2^31 tokens."""
+    cfg = wl.C5
+    gi = wl.gate_inputs(cfg, 0, p_agree=p_agree, tau=tau)
+    for conf_mode in (0, 1):
+        want = P.oracle_gate_compact(gi, conf_mode)
+        sep, fused = P.gpu_gate_compact_all(gi, conf_mode)
+        P.assert_gate_equal(sep, want)
+        P.assert_gate_equal(fused, want)
+    assert want["total_tokens"] > 2 ** 31 or want["n_survivors"] < 2 ** 17
+
+
+@pytest.mark.parametrize("E", [1, 2, 3, 4, 5, 6, 7, 8, 9, 13, 16, 32])
+def test_every_expert_count_and_ragged_sizes(E):
+    g = np.random.default_rng(100 + E)
+    for Q in (1, 31, 255, 256, 257, 1023, 1025, 4097, 70001):
+        a = g.integers(-3, 4, size=(Q, E), dtype=np.int32)
+        w = (g.integers(0, 1 << 24, size=(Q, E)).astype(np.float64) * 2.0 ** -24).astype(np.float32)
+        ctx = g.integers(0, 50000, size=Q, dtype=np.int32)
+        for tau in (0.5, 2.0 / 3.0, 1.0):
+            gi = wl.GateInputs(a, w, ctx, tau, E)
+            for conf_mode in (0, 1):
+                want = P.oracle_gate_compact(gi, conf_mode)
+                sep, fused = P.gpu_gate_compact_all(gi, conf_mode)
+                P.assert_gate_equal(sep, want)
+                P.assert_gate_equal(fused, want)
+
+
+def test_all_bypass_none_bypass_and_empty():
+    from paper_2606_03014_b200 import mosaic
+    Q, E = 5000, 3
+    a = np.tile(np.array([[4, 4, 4]], np.int32), (Q, 1))
+    ctx = np.arange(1, Q + 1, dtype=np.int32)
+    for tau, S in ((1.0, 0), (1.5, Q)):
+        gi = wl.GateInputs(a, None, ctx, tau, E)
+        want = P.oracle_gate_compact(gi, 0)
+        assert want["n_survivors"] == S
+        sep, fused = P.gpu_gate_compact_all(gi, 0)
+        P.assert_gate_equal(sep, want)
+        P.assert_gate_equal(fused, want)
+    # Q == 0: success, S = 0, cu_seqlens = [0]
+    e8 = torch.empty(0, dtype=torch.uint8, device="cuda")
+    e32 = torch.empty(0, dtype=torch.int32, device="cuda")
+    out = dict(n_survivors=torch.full((1,), 7, dtype=torch.int32, device="cuda"),
+               total_tokens=torch.full((1,), 7, dtype=torch.int64, device="cuda"),
+               max_seqlen=torch.full((1,), 7, dtype=torch.int32, device="cuda"),
+               cu_seqlens=torch.full((1,), 7, dtype=torch.int64, device="cuda"))
+    r = mosaic.compact(e8, e32, out=out)
+    torch.cuda.synchronize()
+    assert (int(r["n_survivors"]), int(r["total_tokens"]), int(r["max_seqlen"]),
+            int(r["cu_seqlens"][0])) == (0, 0, 0, 0)
+
+
+def test_workspace_contents_do_not_matter_and_calls_repeat():
+    """The scan workspace is caller scratch with arbitrary contents; repeated calls on the same
+    buffers give the same answer (no state between calls)."""
+    from paper_2606_03014_b200 import mosaic
+    cfg = wl.C4
+    gi = wl.gate_inputs(cfg, 1, Q=100000)
+    want = P.oracle_gate_compact(gi, 0)
+    a = torch.from_numpy(gi.answers).cuda()
+    cl = torch.from_numpy(gi.ctx_len).cuda()
+    ws = torch.randint(0, 255, (mosaic.compact_workspace_bytes(len(cl)),), dtype=torch.uint8,
+                       device="cuda")
+    for _ in range(3):
+        r = mosaic.gate_compact(a, cl, gi.tau, out=dict(workspace=ws))
+        torch.cuda.synchronize()
+        S = int(r["n_survivors"])
+        assert S == want["n_survivors"]
+        assert np.array_equal(r["survivor_idx"][:S].cpu().numpy(), want["survivor_idx"])
+        assert np.array_equal(r["cu_seqlens"][:S + 1].cpu().numpy(), want["cu_seqlens"])
+        ws.random_(0, 255)
+
+
+def test_too_small_workspace_is_an_error():
+    from paper_2606_03014_b200 import mosaic
+    by = torch.zeros(100000, dtype=torch.uint8, device="cuda")
+    cl = torch.ones(100000, dtype=torch.int32, device="cuda")
+    with pytest.raises(mosaic.MosaicError) as e:
+        mosaic.compact(by, cl, out=dict(workspace=torch.empty(64, dtype=torch.uint8, device="cuda")))
+    assert e.value.status == mosaic.ERR_WORKSPACE_TOO_SMALL
