@@ -1,0 +1,387 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the confidence-gated aggregator stage (MOSAIC, Alg. 1) on B200.
+
+A "step" is one pass of the whole hot path over one batch of BASELINE.json configs[1] (C2):
+mosaic_gate_compact over the Q questions, then mosaic_agg_prefill_attn over the survivors'
+packed contexts.  `value` = algorithmic attention FLOPs (4*Hq*D*sum_s L_s(L_s+1)/2, causal pairs
+only) of all ranks / the max-over-ranks device time of the timed steps, inputs resident in HBM.
+`e2e` = the same through mosaic_stage_host from pinned HOST buffers (H2D + D2H inside the timed
+region).  `roofline` is the attention kernel alone (CUDA events around its launches) against the
+measured dense-bf16 peak; `gate` is the gate+compaction kernel on configs[4] (2^20 questions,
+E = 8, weighted confidences) against the measured HBM copy bandwidth, L2-cold by rotating buffer
+sets.  `cpu_baseline` times the fp64 oracle on a bounded row sample of the same workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "gated agg-prefill attn TFLOP/s"
+UNIT = "TFLOP/s"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0}
+
+
+def peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return d, "measured (MEASURED_PEAKS.json)"
+    return dict(FALLBACK_PEAKS), "fallback (B200_PROFILING.md)"
+
+
+def attn_flops(lengths, Hq, D) -> float:
+    L = np.asarray(lengths, np.float64)
+    return float(4.0 * Hq * D * np.sum(L * (L + 1.0) / 2.0))
+
+
+def gate_bytes_per_query(E, weighted, survive_frac):
+    """Algorithmic bytes of the fused gate+compaction pass (kernel G): answers (+
+    weights) + ctx_len read; mode, conf, bypass written; survivor_idx + cu_seqlens per survivor."""
+    return 4 * E * (2 if weighted else 1) + 4 + (4 + 4 + 1) + survive_frac * (4 + 8)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.split(", ") for r in Path(self.f.name).read_text().splitlines() if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.strip().lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(np.max(mx)) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def bf16_bits(t):
+    import torch
+    return t.detach().cpu().contiguous().view(torch.int16).numpy().view(np.uint16)
+
+
+# ------------------------------------------------------------------------------ reference arm
+_ORACLE_INPUTS = {}
+
+
+def oracle_inputs(cfg, seed):
+    """Seeded inputs of the workload as numpy arrays for the oracle (generated once per process)."""
+    if (cfg.config_id, seed) not in _ORACLE_INPUTS:
+        import oracle
+        from paper_2606_03014_b200 import workloads as wl
+        gi = wl.gate_inputs(cfg, seed)
+        oc = oracle.compact(oracle.gate(gi.answers, gi.tau)["bypass"], gi.ctx_len)
+        cu = oc["cu_seqlens"]
+        q, k, v = wl.qkv(cfg, seed, int(cu[-1]))
+        _ORACLE_INPUTS[(cfg.config_id, seed)] = (gi, cu, bf16_bits(q), bf16_bits(k), bf16_bits(v))
+    return _ORACLE_INPUTS[(cfg.config_id, seed)]
+
+
+def oracle_sample(cfg, seed, budget_rows):
+    """A bounded sample of the workload for the CPU oracle: the whole gate + compaction, and
+    `budget_rows` random attention rows (plus the tile / sequence edge rows) of the survivors'
+    batch.  Returns (flops, seconds, threads, description)."""
+    import oracle
+    from paper_2606_03014_b200 import workloads as wl
+
+    gi, cu, qb, kb, vb = oracle_inputs(cfg, seed)
+    rs, rh, rp = wl.sample_rows(cu, cfg.Hq, cfg.Hkv, seed, cfg.config_id, n_random=budget_rows)
+    t0 = time.perf_counter()
+    og = oracle.gate(gi.answers, gi.tau)
+    oracle.compact(og["bypass"], gi.ctx_len)
+    t_gate = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    oracle.attn_rows(qb, kb, vb, cu, rs, rh, rp, wl.softmax_scale(cfg))
+    t_attn = time.perf_counter() - t0
+    flops = float(4.0 * cfg.D * np.sum(rp.astype(np.float64) + 1.0))
+    desc = (f"oracle gate+compact over all {cfg.Q} questions ({t_gate * 1e3:.2f} ms) + "
+            f"{len(rp)} sampled attention rows of {cfg.name} (tile/sequence edges + random), "
+            f"{flops / 1e9:.1f} GFLOP in {t_attn:.2f} s")
+    return flops, t_gate + t_attn, oracle.num_threads(), desc
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_2606_03014_b200 import workloads as wl
+    cfg = wl.C2
+    for _ in range(args.warmup):
+        oracle_sample(cfg, 0, 64)
+    flops = secs = 0.0
+    threads, desc = 1, ""
+    for _ in range(args.steps):
+        f, t, threads, desc = oracle_sample(cfg, 0, args.ref_rows)
+        flops += f
+        secs += t
+    value = flops / secs / 1e12
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": cfg.name + " (BASELINE.json configs[1])",
+                   "note": "each step = a bounded sample of the workload, see cpu_baseline.sample"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
+                         "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------- product arm
+def bench_gate_c5(torch, mosaic, wl, pk, steps, warmup):
+    """Gate + compaction on configs[4] (2^20 questions, E = 8, weighted confidences, p = 0.6,
+    tau = 0.75), L2-cold: 4 disjoint buffer sets (> 2x the 126 MB L2) used round-robin."""
+    cfg = wl.C5
+    gi = wl.gate_inputs(cfg, 0)
+    nsets = 4
+    sets = []
+    for _ in range(nsets):
+        a = torch.from_numpy(gi.answers).cuda()
+        w = torch.from_numpy(gi.expert_conf).cuda()
+        cl = torch.from_numpy(gi.ctx_len).cuda()
+        out = mosaic.gate_compact(a, cl, gi.tau, w, mosaic.CONF_WEIGHTED)
+        sets.append((a, w, cl, out))
+    torch.cuda.synchronize()
+    S = int(sets[0][3]["n_survivors"])
+    bytes_per_call = gate_bytes_per_query(cfg.E, True, S / cfg.Q) * cfg.Q
+
+    def call(i):
+        a, w, cl, out = sets[i % nsets]
+        mosaic.gate_compact(a, cl, gi.tau, w, mosaic.CONF_WEIGHTED, out=out)
+
+    for i in range(warmup):
+        call(i)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in range(steps)]
+    torch.cuda.synchronize()
+    for i, (e0, e1) in enumerate(evs):
+        e0.record()
+        call(i)
+        e1.record()
+    torch.cuda.synchronize()
+    ms = np.array([e0.elapsed_time(e1) for e0, e1 in evs])
+    t = float(np.mean(ms)) * 1e-3
+    gbs = bytes_per_call / t / 1e9
+    return {"workload": "C5-large-sweep gate+compaction: Q=2^20, E=8, weighted conf, p=0.6, tau=0.75",
+            "call": "mosaic_gate_compact (memset + 1 kernel)", "mqueries_per_s": cfg.Q / t / 1e6,
+            "us_per_call": t * 1e6, "us_best": float(ms.min()) * 1e3, "survivors": S,
+            "l2": "cold: 4 buffer sets (~93 MB each) used round-robin",
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                         "frac": gbs / pk["hbm_gbs"], "traffic": None,
+                         "algorithmic_bytes": bytes_per_call}}
+
+
+def run_product(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2606_03014_b200 import mosaic
+    from paper_2606_03014_b200 import workloads as wl
+
+    mosaic.load()  # fails loudly when the CUDA library is missing: there is no fallback
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    pk, pk_src = peaks()
+    cfg = wl.C2
+    seed = rank  # weak scaling: every rank gates and attends its own batch, no collective
+    gi = wl.gate_inputs(cfg, seed)
+    a = torch.from_numpy(gi.answers).cuda()
+    cl = torch.from_numpy(gi.ctx_len).cuda()
+    gout = mosaic.gate_compact(a, cl, gi.tau)
+    torch.cuda.synchronize()
+    S, T, max_len = int(gout["n_survivors"]), int(gout["total_tokens"]), int(gout["max_seqlen"])
+    cu_host = gout["cu_seqlens"][:S + 1].cpu().numpy()
+    lengths = np.diff(cu_host)
+    flops = attn_flops(lengths, cfg.Hq, cfg.D)
+    q, k, v = wl.qkv(cfg, seed, T, device="cuda")
+    o = torch.empty_like(q)
+    lse = torch.empty((cfg.Hq, T), dtype=torch.float32, device="cuda")
+    ws = torch.empty(mosaic.attn_workspace_bytes(S, T, cfg.Hq, cfg.Hkv, cfg.D), dtype=torch.uint8,
+                     device="cuda")
+    scale = wl.softmax_scale(cfg)
+    ev_attn = []
+
+    def step(timed):
+        mosaic.gate_compact(a, cl, gi.tau, out=gout)
+        if timed:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+        mosaic.agg_prefill_attn(q, k, v, gout["cu_seqlens"], S, max_len, scale, o=o, lse=lse,
+                                workspace=ws)
+        if timed:
+            e1.record()
+            ev_attn.append((e0, e1))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step(False)
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    l0 = mosaic.kernel_launch_count()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for _ in range(args.steps):
+        step(True)
+    t1.record()
+    barrier()
+    launches = mosaic.kernel_launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    secs = t0.elapsed_time(t1) * 1e-3
+    attn_ms = float(np.mean([e0.elapsed_time(e1) for e0, e1 in ev_attn]))
+    tot = torch.tensor([secs, flops * args.steps], dtype=torch.float64, device="cuda")
+    if world > 1:
+        mx = tot.clone()
+        dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        secs_max, flops_all = float(mx[0]), float(tot[1])
+    else:
+        secs_max, flops_all = secs, float(tot[1])
+    value = flops_all / secs_max / 1e12
+
+    # ---- end to end through the host-buffer call (pinned host memory, copies timed) ----------
+    qh, kh, vh = (t.cpu().pin_memory() for t in (q, k, v))
+    ah, clh = torch.from_numpy(gi.answers).pin_memory(), torch.from_numpy(gi.ctx_len).pin_memory()
+    del q, k, v, o, lse
+    torch.cuda.empty_cache()
+    out_h = {"o": torch.empty((T, cfg.Hq, cfg.D), dtype=torch.bfloat16).pin_memory(),
+             "lse": torch.empty(cfg.Hq * T, dtype=torch.float32).pin_memory(),
+             "mode": torch.empty(cfg.Q, dtype=torch.int32).pin_memory(),
+             "conf": torch.empty(cfg.Q, dtype=torch.float32).pin_memory(),
+             "bypass": torch.empty(cfg.Q, dtype=torch.uint8).pin_memory()}
+    arena = torch.empty(mosaic.stage_host_arena_bytes(cfg.Q, cfg.E, T, cfg.Hq, cfg.Hkv, cfg.D),
+                        dtype=torch.uint8, device="cuda")
+    e2e_steps = max(3, min(args.steps, 10))
+    for _ in range(2):
+        mosaic.stage_host(ah, None, clh, gi.tau, 0, qh, kh, vh, scale, out_h=out_h, arena=arena)
+    barrier()
+    w0 = time.perf_counter()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(e2e_steps):
+        mosaic.stage_host(ah, None, clh, gi.tau, 0, qh, kh, vh, scale, out_h=out_h, arena=arena)
+    e1.record()
+    barrier()
+    e2e_secs = max(e0.elapsed_time(e1) * 1e-3, 0.0)
+    e2e_wall = time.perf_counter() - w0
+    tt = torch.tensor([e2e_secs], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    e2e_value = flops_all / args.steps * e2e_steps / float(tt[0]) / 1e12
+    h2d = gi.answers.nbytes + gi.ctx_len.nbytes + (qh.numel() + kh.numel() + vh.numel()) * 2
+    d2h = (16 + cfg.Q * 9 + S * 4 + (S + 1) * 8 + T * cfg.Hq * cfg.D * 2 + T * cfg.Hq * 4)
+    del arena
+    torch.cuda.empty_cache()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    gate_info = bench_gate_c5(torch, mosaic, wl, pk, steps=40, warmup=8)
+    f, t, threads, desc = oracle_sample(cfg, 0, args.cpu_rows)
+    attn_tflops = flops / (attn_ms * 1e-3) / 1e12
+    traffic = None
+    tj = ROOT / "profiles" / "traffic.json"
+    if tj.exists():
+        traffic = json.loads(tj.read_text()).get("attn_fwd_dram_bytes_per_launch")
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": secs_max / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic",
+        "config": {"workload": cfg.name + " (BASELINE.json configs[1])", "Q": cfg.Q, "E": cfg.E,
+                   "tau": cfg.tau, "survivors": S, "total_tokens": T, "max_seqlen": max_len,
+                   "Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D, "per_rank_seed": "rank",
+                   "algorithmic_tflop_per_step": flops / 1e12,
+                   "l2": "inputs larger than L2 (Q+K+V+O = %.2f GB per step)" %
+                         ((2 * T * cfg.Hq + 2 * T * cfg.Hkv) * cfg.D * 2 / 1e9),
+                   "peaks": pk_src},
+        "roofline": {"bound": "tensor", "achieved": attn_tflops, "peak": pk["bf16_tflops"],
+                     "unit": "TFLOP/s", "frac": attn_tflops / pk["bf16_tflops"],
+                     "traffic": traffic, "kernel": "attn_fwd (+ schedule_kernel)",
+                     "ms_per_launch": attn_ms, "peak_kind": "burst bf16_tflops"},
+        "gate": gate_info,
+        "cpu_baseline": {"value": f / t / 1e12, "unit": UNIT, "cores": threads, "kind": "oracle",
+                         "sample": desc},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
+                "ms_per_step": float(tt[0]) / e2e_steps * 1e3,
+                "wall_ms_per_step": e2e_wall / e2e_steps * 1e3,
+                "call": "mosaic_stage_host (pinned host buffers)"},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="mosaic", choices=["mosaic", "reference"])
+    ap.add_argument("--ref-rows", type=int, default=4096, help="reference arm: rows per step")
+    ap.add_argument("--cpu-rows", type=int, default=524288, help="cpu_baseline: sampled rows")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_product(args)
+
+
+if __name__ == "__main__":
+    main()
