@@ -7,10 +7,13 @@
 //   mosaic_compact       DO_COMPACT         -- single-pass scan (decoupled look-back)
 //   mosaic_gate_compact  DO_GATE|DO_COMPACT -- both in one pass over HBM
 //
-// HBM-bound: every input byte is read once with 16-byte loads where the
-// row width allows, outputs are written once, coalesced.  A tile is THREADS x ITEMS questions in
-// a striped arrangement (question = tile_base + item * THREADS + thread) so a warp's loads and
-// its compacted stores are both contiguous.
+// HBM-bound.  A tile is kThreads x items questions in a striped
+// arrangement (question = tile_base + item * kThreads + thread) so that a warp's loads and its
+// compacted stores are both contiguous.  `items` is chosen on the host so that the whole grid is
+// ONE wave of co-resident blocks (2 per SM) whenever Q allows: every block streams its rows
+// (16- or 32-byte loads, several rows in flight per thread), keeps only (survived, ctx_len) per
+// question in registers, and the scan costs one look-back round at the end of the block instead
+// of one per small tile.
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
@@ -22,49 +25,62 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
-constexpr int kMinTile = kThreads;  // smallest tile any instantiation uses (ITEMS == 1)
+constexpr int kMaxItems = 16;     // questions per thread, specialised E (<= 8)
+constexpr int kMaxItemsWide = 4;  // ... generic E (<= 32): rows live in 2 x 32 registers
+constexpr int kBlocksPerSM = 2;
 
 using u64 = unsigned long long;
 
-// Scan state of one tile: two independent words, each carrying its own 2-bit status in bits
-// 62..63 (0 = not written, 1 = tile aggregate, 2 = inclusive prefix) so that a relaxed 64-bit
-// load always sees a value together with its status.
+// Scan state of one tile, 16 bytes, written and read with single 128-bit accesses:
+//   lo = status(2) | max ctx_len of survivors (31) | survivor count (31)
+//   hi = status(2) | survivors' context tokens (62)
+// status 0 = not written, 1 = this tile's aggregate, 2 = inclusive prefix over tiles 0..this.
+// A reader accepts a pair only when both words carry the same non-zero status.
 struct alignas(16) TileState {
-    u64 count;   // survivors
-    u64 tokens;  // context tokens of the survivors
+    u64 lo, hi;
 };
-constexpr u64 kValueMask = (1ull << 62) - 1;
 constexpr u64 kAggregate = 1ull << 62;
 constexpr u64 kPrefix = 2ull << 62;
+constexpr u64 kMask62 = (1ull << 62) - 1;
+constexpr u64 kMask31 = (1ull << 31) - 1;
 
 struct alignas(16) ScanHeader {
-    unsigned int ticket;    // next tile id (tiles are handed out in start order)
-    unsigned int finished;  // tiles done
-    int max_len;            // running max of the survivors' ctx_len
-    int pad;
+    unsigned int ticket;  // next tile id (tiles are handed out in start order)
+    unsigned int pad[3];
 };
 
-__device__ __forceinline__ u64 ld_relaxed(const u64* p) {
-    u64 v;
-    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
+struct Partial {  // the three scanned quantities
+    u64 count, tokens;
+    int max_len;
+};
+
+__device__ __forceinline__ u64 pack_lo(u64 status, const Partial& p) {
+    return status | ((u64)(uint32_t)p.max_len << 31) | p.count;
 }
-__device__ __forceinline__ void st_relaxed(u64* p, u64 v) {
-    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+__device__ __forceinline__ void ld_state(const TileState* s, u64& lo, u64& hi) {
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(lo), "=l"(hi) : "l"(s) : "memory");
+}
+__device__ __forceinline__ void st_state(TileState* s, u64 lo, u64 hi) {
+    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(s), "l"(lo), "l"(hi) : "memory");
 }
 
-__device__ __forceinline__ u64 warp_sum(u64 v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-// Row loads: 16-byte vectors when the row width allows (rows start 16-byte aligned when
-// E % 4 == 0 because the base pointer is), 8-byte for E % 2 == 0, scalar otherwise.
+// Row loads.  Rows start 16-byte aligned when E % 4 == 0 (32-byte when E % 8 == 0) because the
+// base pointer is; 32-byte rows use one 256-bit load, streamed past L1.
 template <int E_T, int EM, typename T>
 __device__ __forceinline__ void load_row(const T* __restrict__ base, int64_t q, int E, T (&r)[EM]) {
     static_assert(sizeof(T) == 4, "");
-    if constexpr (E_T != 0 && E_T % 4 == 0) {
+    if constexpr (E_T != 0 && E_T % 8 == 0) {
+#pragma unroll
+        for (int i = 0; i < E_T / 8; ++i) {
+            uint32_t v[8];
+            asm volatile("ld.global.nc.L1::no_allocate.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                         : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]),
+                           "=r"(v[6]), "=r"(v[7])
+                         : "l"(base + q * E_T + 8 * i));
+#pragma unroll
+            for (int j = 0; j < 8; ++j) r[8 * i + j] = reinterpret_cast<T&>(v[j]);
+        }
+    } else if constexpr (E_T != 0 && E_T % 4 == 0) {
         const int4* p = reinterpret_cast<const int4*>(base + q * E_T);
 #pragma unroll
         for (int i = 0; i < E_T / 4; ++i) {
@@ -90,25 +106,90 @@ __device__ __forceinline__ void load_row(const T* __restrict__ base, int64_t q, 
     }
 }
 
+// Sorting networks with the optimal comparator counts (1, 3, 5, 9, 12, 16, 19) for 2..8 labels.
+__device__ __forceinline__ void cmp_swap(int32_t& x, int32_t& y) {
+    const int32_t lo = min(x, y), hi = max(x, y);
+    x = lo;
+    y = hi;
+}
+template <int N>
+__device__ __forceinline__ void sort_labels(int32_t (&s)[N]) {
+    static_assert(N >= 1 && N <= 8, "");
+    if constexpr (N == 2) {
+        cmp_swap(s[0], s[1]);
+    }
+    if constexpr (N == 3) {
+        cmp_swap(s[0], s[2]); cmp_swap(s[0], s[1]); cmp_swap(s[1], s[2]);
+    }
+    if constexpr (N == 4) {
+        cmp_swap(s[0], s[2]); cmp_swap(s[1], s[3]); cmp_swap(s[0], s[1]); cmp_swap(s[2], s[3]);
+        cmp_swap(s[1], s[2]);
+    }
+    if constexpr (N == 5) {
+        cmp_swap(s[0], s[3]); cmp_swap(s[1], s[4]); cmp_swap(s[0], s[2]); cmp_swap(s[1], s[3]);
+        cmp_swap(s[0], s[1]); cmp_swap(s[2], s[4]); cmp_swap(s[1], s[2]); cmp_swap(s[3], s[4]);
+        cmp_swap(s[2], s[3]);
+    }
+    if constexpr (N == 6) {
+        cmp_swap(s[0], s[5]); cmp_swap(s[1], s[3]); cmp_swap(s[2], s[4]); cmp_swap(s[1], s[2]);
+        cmp_swap(s[3], s[4]); cmp_swap(s[0], s[3]); cmp_swap(s[2], s[5]); cmp_swap(s[0], s[1]);
+        cmp_swap(s[2], s[3]); cmp_swap(s[4], s[5]); cmp_swap(s[1], s[2]); cmp_swap(s[3], s[4]);
+    }
+    if constexpr (N == 7) {
+        cmp_swap(s[0], s[6]); cmp_swap(s[2], s[3]); cmp_swap(s[4], s[5]); cmp_swap(s[0], s[2]);
+        cmp_swap(s[1], s[4]); cmp_swap(s[3], s[6]); cmp_swap(s[0], s[1]); cmp_swap(s[2], s[5]);
+        cmp_swap(s[3], s[4]); cmp_swap(s[1], s[2]); cmp_swap(s[4], s[6]); cmp_swap(s[2], s[3]);
+        cmp_swap(s[4], s[5]); cmp_swap(s[1], s[2]); cmp_swap(s[3], s[4]); cmp_swap(s[5], s[6]);
+    }
+    if constexpr (N == 8) {
+        cmp_swap(s[0], s[2]); cmp_swap(s[1], s[3]); cmp_swap(s[4], s[6]); cmp_swap(s[5], s[7]);
+        cmp_swap(s[0], s[4]); cmp_swap(s[1], s[5]); cmp_swap(s[2], s[6]); cmp_swap(s[3], s[7]);
+        cmp_swap(s[0], s[1]); cmp_swap(s[2], s[3]); cmp_swap(s[4], s[5]); cmp_swap(s[6], s[7]);
+        cmp_swap(s[2], s[4]); cmp_swap(s[3], s[5]); cmp_swap(s[1], s[4]); cmp_swap(s[3], s[6]);
+        cmp_swap(s[1], s[2]); cmp_swap(s[3], s[4]); cmp_swap(s[5], s[6]);
+    }
+}
+
 // Alg. 1 lines 2-4 for one question.  Same decisions, in the same precision, as
-// the definition: c* by counting, mode = smallest label among those reaching c* (reading G-2),
-// agree = fl32(c*)/fl32(E) (one IEEE division, reading G-4), weighted share in binary64 in
-// expert order (reading G-10), bypass = conf >= tau in fp32 (">=").
-template <int EM, int CONF>
+// the definition: c* = the largest number of equal labels, mode = smallest label among those
+// reaching c* (reading G-2), agree = fl32(c*)/fl32(E) (one IEEE division, reading G-4), weighted
+// share in binary64 in expert order (reading G-10), bypass = conf >= tau in fp32 (">=").
+// SORTED (E known at compile time, <= 8): the labels go through a sorting network and the
+// plurality is the longest run, first (= smallest label) run winning ties; otherwise every label
+// is counted against every other.
+template <int EM, int CONF, bool SORTED>
 __device__ __forceinline__ void gate_row(const int32_t (&a)[EM], const float (&w)[EM], int E,
                                          float tau, int32_t& mode, int32_t& count, float& agree,
                                          float& conf, bool& bypass) {
     int32_t c_star = 0, md = 0;
+    if constexpr (SORTED) {
+        int32_t s[EM];
 #pragma unroll
-    for (int i = 0; i < EM; ++i) {
-        if (i < E) {
-            int32_t n = 0;
+        for (int i = 0; i < EM; ++i) s[i] = a[i];
+        sort_labels<EM>(s);
+        int32_t run = 1;
+        c_star = 1;
+        md = s[0];
 #pragma unroll
-            for (int j = 0; j < EM; ++j)
-                if (j < E) n += (a[j] == a[i]) ? 1 : 0;
-            if (n > c_star || (n == c_star && a[i] < md)) {
-                c_star = n;
-                md = a[i];
+        for (int i = 1; i < EM; ++i) {
+            run = (s[i] == s[i - 1]) ? run + 1 : 1;
+            if (run > c_star) {
+                c_star = run;
+                md = s[i];
+            }
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < EM; ++i) {
+            if (i < E) {
+                int32_t n = 0;
+#pragma unroll
+                for (int j = 0; j < EM; ++j)
+                    if (j < E) n += (a[j] == a[i]) ? 1 : 0;
+                if (n > c_star || (n == c_star && a[i] < md)) {
+                    c_star = n;
+                    md = a[i];
+                }
             }
         }
     }
@@ -152,221 +233,278 @@ struct GateArgs {
     ScanHeader* header;
     TileState* tiles;
     unsigned int num_tiles;
+    int items;  // questions per thread in this launch
 };
 
-// Sum, over the tiles before `tile`, of both scanned quantities (decoupled look-back: walk the
-// predecessors 32 at a time, adding aggregates until an inclusive prefix is met).  The two words
-// are walked in lockstep but finish independently.  Whole warp calls; result in every lane.
-__device__ __forceinline__ void look_back(const TileState* tiles, int tile, int lane, u64& count,
-                                          u64& tokens) {
-    u64 acc_c = 0, acc_t = 0;
-    bool done_c = false, done_t = false;
-    for (int base = tile - 1; !(done_c && done_t); base -= 32) {
-        const int idx = base - lane;
-        u64 wc = kPrefix, wt = kPrefix;  // "tile -1": prefix 0
-        if (idx >= 0) {
-            const u64* pc = &tiles[idx].count;
-            const u64* pt = &tiles[idx].tokens;
-            for (;;) {
-                wc = ld_relaxed(pc);
-                wt = ld_relaxed(pt);
-                if ((wc >> 62) != 0 && (wt >> 62) != 0) break;
-                __nanosleep(20);
+// Combined (count, tokens, max) of the tiles before `tile` (decoupled look-back).  Warp 0 walks
+// the predecessors 256 at a time, 8 per lane, nearest first: each lane adds its entries up to and
+// including its first inclusive prefix; lanes before the first lane that met a prefix count in
+// full, that lane counts its partial sum, later lanes do not count.  With the grid a single wave
+// of <= 296 tiles this is one round of loads.  Whole warp calls; result in every lane.
+__device__ __forceinline__ Partial look_back(const TileState* tiles, int tile, int lane) {
+    constexpr int W = 8;
+    Partial acc{0, 0, 0};
+    bool done = false;
+    for (int base = tile - 1; !done; base -= 32 * W) {
+        u64 lo[W], hi[W];
+#pragma unroll
+        for (int j = 0; j < W; ++j) {
+            const int idx = base - (lane * W + j);
+            lo[j] = hi[j] = kPrefix;  // "tile -1": prefix of nothing
+            if (idx >= 0) ld_state(tiles + idx, lo[j], hi[j]);
+        }
+        Partial mine{0, 0, 0};
+        bool met = false;
+#pragma unroll
+        for (int j = 0; j < W; ++j) {
+            const int idx = base - (lane * W + j);
+            if (idx >= 0) {
+                while ((lo[j] >> 62) == 0 || (lo[j] >> 62) != (hi[j] >> 62))
+                    ld_state(tiles + idx, lo[j], hi[j]);
+            }
+            if (!met) {
+                mine.count += lo[j] & kMask31;
+                mine.tokens += hi[j] & kMask62;
+                mine.max_len = max(mine.max_len, (int)((lo[j] >> 31) & kMask31));
+                met = (lo[j] >> 62) == 2;
             }
         }
         __syncwarp();
-        if (!done_c) {
-            const unsigned pm = __ballot_sync(0xffffffffu, (wc >> 62) == 2);
-            const int first = pm ? (__ffs(pm) - 1) : 31;
-            acc_c += warp_sum(lane <= first ? (wc & kValueMask) : 0ull);
-            done_c = pm != 0;
+        const unsigned pm = __ballot_sync(0xffffffffu, met);
+        const int first = pm ? (__ffs(pm) - 1) : 31;
+        if (lane > first) mine = Partial{0, 0, 0};
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            mine.count += __shfl_xor_sync(0xffffffffu, mine.count, o);
+            mine.tokens += __shfl_xor_sync(0xffffffffu, mine.tokens, o);
+            mine.max_len = max(mine.max_len, __shfl_xor_sync(0xffffffffu, mine.max_len, o));
         }
-        if (!done_t) {
-            const unsigned pm = __ballot_sync(0xffffffffu, (wt >> 62) == 2);
-            const int first = pm ? (__ffs(pm) - 1) : 31;
-            acc_t += warp_sum(lane <= first ? (wt & kValueMask) : 0ull);
-            done_t = pm != 0;
-        }
+        acc.count += mine.count;
+        acc.tokens += mine.tokens;
+        acc.max_len = max(acc.max_len, mine.max_len);
+        done = pm != 0;
     }
-    count = acc_c;
-    tokens = acc_t;
+    return acc;
 }
 
-template <int E_T, int CONF, bool DO_GATE, bool DO_COMPACT, int ITEMS>
-__global__ void __launch_bounds__(kThreads) gate_compact_kernel(const GateArgs p) {
+// Shared memory of one block: per-question (survived ? ctx_len : -1) in striped order, and the
+// per-(item, warp) partials of the scan.
+template <int MAXI>
+struct GateSmem {
+    int len[MAXI * kThreads];
+    unsigned int part_count[MAXI * kWarps];  // survivors of (item, warp)  -> exclusive offsets
+    u64 part_tokens[MAXI * kWarps];          // their context tokens       -> exclusive offsets
+    u64 base_count, base_tokens;             // the tile's exclusive prefix
+    int warp_max[kWarps];
+    unsigned int tile;
+};
+
+template <int E_T, int CONF, bool DO_GATE, bool DO_COMPACT, int MAXI, int BATCH>
+__global__ void __launch_bounds__(kThreads, kBlocksPerSM) gate_compact_kernel(const GateArgs p) {
     constexpr int EM = DO_GATE ? (E_T ? E_T : MOSAIC_MAX_EXPERTS) : 1;
-    constexpr int TILE = kThreads * ITEMS;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int E = E_T ? E_T : p.E;
+    const int items = p.items;
 
-    __shared__ unsigned int s_tile;
-    __shared__ u64 s_wcount[ITEMS * kWarps];  // per (item, warp) survivor counts -> exclusive offsets
-    __shared__ u64 s_wtok[ITEMS * kWarps];    // per (item, warp) token sums      -> exclusive offsets
-    __shared__ u64 s_base[2];                 // the tile's exclusive prefix (count, tokens)
-    __shared__ int s_max;
+    __shared__ GateSmem<DO_COMPACT ? MAXI : 1> sm;
 
     unsigned int tile = blockIdx.x;
     if constexpr (DO_COMPACT) {
-        if (tid == 0) {
-            s_tile = atomicAdd(&p.header->ticket, 1u);
-            s_max = 0;
-        }
+        if (tid == 0) sm.tile = atomicAdd(&p.header->ticket, 1u);
         __syncthreads();
-        tile = s_tile;
+        tile = sm.tile;
     }
-    const int64_t q0 = (int64_t)tile * TILE;
+    const int64_t q0 = (int64_t)tile * kThreads * items;
+    int my_max = 0;
 
-    bool surv[ITEMS];
-    int32_t len[ITEMS];
-
-    // ---- G1-G3: vote, confidence, threshold ---------------------------------------------------
-    if constexpr (DO_GATE) {
-        int32_t a[ITEMS][EM];
-        float w[ITEMS][EM];
+    // ---- G1-G3 (vote, confidence, threshold), BATCH questions per thread in flight ---------------
+    for (int it0 = 0; it0 < items; it0 += BATCH) {
+        bool valid[BATCH], surv[BATCH];
+        int32_t len[BATCH];
+        if constexpr (DO_GATE) {
+            int32_t a[BATCH][EM];
+            float w[BATCH][EM];
 #pragma unroll
-        for (int k = 0; k < ITEMS; ++k) {
-            const int64_t q = q0 + k * kThreads + tid;
-            if (q < p.Q) {
-                load_row<E_T, EM>(p.answers, q, E, a[k]);
-                if constexpr (CONF == MOSAIC_CONF_WEIGHTED)
-                    load_row<E_T, EM>(p.expert_conf, q, E, w[k]);
+            for (int k = 0; k < BATCH; ++k) {
+                const int64_t q = q0 + (int64_t)(it0 + k) * kThreads + tid;
+                valid[k] = (it0 + k < items) && (q < p.Q);
+                if (valid[k]) {
+                    load_row<E_T, EM>(p.answers, q, E, a[k]);
+                    if constexpr (CONF == MOSAIC_CONF_WEIGHTED)
+                        load_row<E_T, EM>(p.expert_conf, q, E, w[k]);
+                    if constexpr (DO_COMPACT) len[k] = __ldg(p.ctx_len + q);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < BATCH; ++k) {
+                const int64_t q = q0 + (int64_t)(it0 + k) * kThreads + tid;
+                surv[k] = false;
+                if (valid[k]) {
+                    int32_t mode, count;
+                    float agree, conf;
+                    bool bypass;
+                    gate_row<EM, CONF, (E_T != 0)>(a[k], w[k], E, p.tau, mode, count, agree, conf, bypass);
+                    if (p.mode_out) __stcs(p.mode_out + q, mode);
+                    if (p.count_out) __stcs(p.count_out + q, count);
+                    if (p.agree_out) __stcs(p.agree_out + q, agree);
+                    if (p.conf_out) __stcs(p.conf_out + q, conf);
+                    if (p.bypass_out) p.bypass_out[q] = bypass ? 1 : 0;
+                    surv[k] = !bypass;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < BATCH; ++k) {
+                const int64_t q = q0 + (int64_t)(it0 + k) * kThreads + tid;
+                valid[k] = (it0 + k < items) && (q < p.Q);
+                surv[k] = valid[k] ? (__ldg(p.bypass_in + q) == 0) : false;
+                len[k] = valid[k] ? __ldg(p.ctx_len + q) : 0;
             }
         }
         if constexpr (DO_COMPACT) {
+            // per-(item, warp) partials: survivors, their tokens (two 16-bit-half reductions so the
+            // 32-lane sums cannot overflow 32 bits), max length
 #pragma unroll
-            for (int k = 0; k < ITEMS; ++k) {
-                const int64_t q = q0 + k * kThreads + tid;
-                len[k] = (q < p.Q) ? __ldg(p.ctx_len + q) : 0;
+            for (int k = 0; k < BATCH; ++k) {
+                if (it0 + k < items) {
+                    const uint32_t v = surv[k] ? (uint32_t)len[k] : 0u;
+                    sm.len[(it0 + k) * kThreads + tid] = surv[k] ? len[k] : -1;
+                    const unsigned ballot = __ballot_sync(0xffffffffu, surv[k]);
+                    const uint32_t lo = __reduce_add_sync(0xffffffffu, v & 0xffffu);
+                    const uint32_t hi = __reduce_add_sync(0xffffffffu, v >> 16);
+                    my_max = max(my_max, (int)v);
+                    if (lane == 0) {
+                        sm.part_count[(it0 + k) * kWarps + warp] = __popc(ballot);
+                        sm.part_tokens[(it0 + k) * kWarps + warp] = (u64)lo + ((u64)hi << 16);
+                    }
+                }
             }
-        }
-#pragma unroll
-        for (int k = 0; k < ITEMS; ++k) {
-            const int64_t q = q0 + k * kThreads + tid;
-            surv[k] = false;
-            if (q < p.Q) {
-                int32_t mode, count;
-                float agree, conf;
-                bool bypass;
-                gate_row<EM, CONF>(a[k], w[k], E, p.tau, mode, count, agree, conf, bypass);
-                if (p.mode_out) p.mode_out[q] = mode;
-                if (p.count_out) p.count_out[q] = count;
-                if (p.agree_out) p.agree_out[q] = agree;
-                if (p.conf_out) p.conf_out[q] = conf;
-                if (p.bypass_out) p.bypass_out[q] = bypass ? 1 : 0;
-                surv[k] = !bypass;
-            }
-        }
-    } else {
-#pragma unroll
-        for (int k = 0; k < ITEMS; ++k) {
-            const int64_t q = q0 + k * kThreads + tid;
-            surv[k] = (q < p.Q) ? (__ldg(p.bypass_in + q) == 0) : false;
-            len[k] = (q < p.Q) ? __ldg(p.ctx_len + q) : 0;
         }
     }
+
     if constexpr (DO_COMPACT) {
-    // ---- G4-G5: stable compaction and cu_seqlens -------------------------------------------------
-    // Scan order inside the tile is (item, thread): exactly ascending question index.
-    unsigned rank_in_warp[ITEMS];
-    u64 tok_incl[ITEMS];
-    int my_max = 0;
-#pragma unroll
-    for (int k = 0; k < ITEMS; ++k) {
-        const unsigned ballot = __ballot_sync(0xffffffffu, surv[k]);
-        rank_in_warp[k] = __popc(ballot & ((1u << lane) - 1u));
-        u64 v = surv[k] ? (u64)(uint32_t)len[k] : 0ull;
-        if (surv[k]) my_max = max(my_max, len[k]);
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const u64 t = __shfl_up_sync(0xffffffffu, v, o);
-            if (lane >= o) v += t;
-        }
-        tok_incl[k] = v;
-        if (lane == 31) {
-            s_wcount[k * kWarps + warp] = (u64)__popc(ballot);
-            s_wtok[k * kWarps + warp] = v;
-        }
-    }
-    my_max = __reduce_max_sync(0xffffffffu, my_max);
-    if (lane == 0 && my_max > 0) atomicMax(&s_max, my_max);
-    __syncthreads();
+        // ---- G4-G5: stable compaction and cu_seqlens -------------------------------------------
+        // Scan order inside the tile is (item, thread): exactly ascending question index.
+        my_max = __reduce_max_sync(0xffffffffu, my_max);
+        if (lane == 0) sm.warp_max[warp] = my_max;
+        __syncthreads();
 
-    if (warp == 0) {
-        // exclusive scan of the ITEMS*kWarps (<= 32) partials, then the tile's global prefix
-        static_assert(ITEMS * kWarps <= 32, "partials must fit one warp");
-        const bool has = lane < ITEMS * kWarps;
-        const u64 c = has ? s_wcount[lane] : 0ull, t = has ? s_wtok[lane] : 0ull;
-        u64 ci = c, ti = t;
+        if (warp == 0) {
+            // exclusive scan of the items * kWarps (<= 128) partials, 4 consecutive per lane
+            constexpr int PER = (MAXI * kWarps + 31) / 32;
+            const int n_part = items * kWarps;
+            unsigned int c[PER];
+            u64 t[PER];
+            unsigned int csum = 0;
+            u64 tsum = 0;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const u64 cc = __shfl_up_sync(0xffffffffu, ci, o);
-            const u64 tt = __shfl_up_sync(0xffffffffu, ti, o);
-            if (lane >= o) {
-                ci += cc;
-                ti += tt;
+            for (int j = 0; j < PER; ++j) {
+                const int e = lane * PER + j;
+                c[j] = e < n_part ? sm.part_count[e] : 0u;
+                t[j] = e < n_part ? sm.part_tokens[e] : 0ull;
+                csum += c[j];
+                tsum += t[j];
             }
-        }
-        if (has) {
-            s_wcount[lane] = ci - c;
-            s_wtok[lane] = ti - t;
-        }
-        const u64 tile_c = __shfl_sync(0xffffffffu, ci, 31), tile_t = __shfl_sync(0xffffffffu, ti, 31);
-        TileState* me = p.tiles + tile;
-        if (tile == 0) {
-            if (lane == 0) {
-                st_relaxed(&me->count, kPrefix | tile_c);
-                st_relaxed(&me->tokens, kPrefix | tile_t);
-                s_base[0] = 0;
-                s_base[1] = 0;
-                p.cu_seqlens[0] = 0;
-            }
-        } else {
-            if (lane == 0) {
-                st_relaxed(&me->count, kAggregate | tile_c);
-                st_relaxed(&me->tokens, kAggregate | tile_t);
-            }
-            u64 pc, pt;
-            look_back(p.tiles, (int)tile, lane, pc, pt);
-            if (lane == 0) {
-                st_relaxed(&me->count, kPrefix | (pc + tile_c));
-                st_relaxed(&me->tokens, kPrefix | (pt + tile_t));
-                s_base[0] = pc;
-                s_base[1] = pt;
-            }
-        }
-        if (lane == 0 && tile == p.num_tiles - 1) {
-            *p.n_survivors = (int32_t)(s_base[0] + tile_c);
-            *p.total_tokens = (int64_t)(s_base[1] + tile_t);
-        }
-    }
-    __syncthreads();
-
-    const u64 base_c = s_base[0], base_t = s_base[1];
+            unsigned int ci = csum;
+            u64 ti = tsum;
 #pragma unroll
-    for (int k = 0; k < ITEMS; ++k) {
-        if (surv[k]) {
-            const u64 r = base_c + s_wcount[k * kWarps + warp] + rank_in_warp[k];
-            p.survivor_idx[r] = (int32_t)(q0 + k * kThreads + tid);
-            p.cu_seqlens[r + 1] = (int64_t)(base_t + s_wtok[k * kWarps + warp] + tok_incl[k]);
-        }
-    }
+            for (int o = 1; o < 32; o <<= 1) {
+                const unsigned int cc = __shfl_up_sync(0xffffffffu, ci, o);
+                const u64 tt = __shfl_up_sync(0xffffffffu, ti, o);
+                if (lane >= o) {
+                    ci += cc;
+                    ti += tt;
+                }
+            }
+            unsigned int cx = ci - csum;
+            u64 tx = ti - tsum;
+#pragma unroll
+            for (int j = 0; j < PER; ++j) {
+                const int e = lane * PER + j;
+                if (e < n_part) {
+                    sm.part_count[e] = cx;
+                    sm.part_tokens[e] = tx;
+                }
+                cx += c[j];
+                tx += t[j];
+            }
+            Partial mine;
+            mine.count = __shfl_sync(0xffffffffu, ci, 31);
+            mine.tokens = __shfl_sync(0xffffffffu, ti, 31);
+            mine.max_len = __reduce_max_sync(0xffffffffu, lane < kWarps ? sm.warp_max[lane] : 0);
 
-    if (tid == 0) {
-        if (s_max > 0) atomicMax(&p.header->max_len, s_max);
-        __threadfence();
-        const unsigned done = atomicAdd(&p.header->finished, 1u);
-        if (done == p.num_tiles - 1) {
-            __threadfence();
-            *p.max_seqlen = *reinterpret_cast<volatile int*>(&p.header->max_len);
+            TileState* me = p.tiles + tile;
+            Partial before{0, 0, 0};
+            if (tile != 0) {
+                if (lane == 0) st_state(me, pack_lo(kAggregate, mine), kAggregate | mine.tokens);
+                before = look_back(p.tiles, (int)tile, lane);
+            }
+            Partial incl{before.count + mine.count, before.tokens + mine.tokens,
+                         max(before.max_len, mine.max_len)};
+            if (lane == 0) {
+                st_state(me, pack_lo(kPrefix, incl), kPrefix | incl.tokens);
+                sm.base_count = before.count;
+                sm.base_tokens = before.tokens;
+                if (tile == 0) p.cu_seqlens[0] = 0;
+                if (tile == p.num_tiles - 1) {
+                    *p.n_survivors = (int32_t)incl.count;
+                    *p.total_tokens = (int64_t)incl.tokens;
+                    *p.max_seqlen = incl.max_len;
+                }
+            }
+        }
+        __syncthreads();
+
+        const u64 base_c = sm.base_count, base_t = sm.base_tokens;
+        for (int k = 0; k < items; ++k) {
+            const int v = sm.len[k * kThreads + tid];
+            const bool s = v >= 0;
+            const unsigned ballot = __ballot_sync(0xffffffffu, s);
+            if (ballot == 0) continue;
+            const unsigned rank = __popc(ballot & ((1u << lane) - 1u));
+            u64 incl;
+            const uint32_t vv = s ? (uint32_t)v : 0u;
+            if (__reduce_max_sync(0xffffffffu, vv) < (1u << 26)) {  // 32 lanes cannot overflow
+                uint32_t x = vv;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+                    if (lane >= o) x += y;
+                }
+                incl = x;
+            } else {
+                u64 x = vv;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const u64 y = __shfl_up_sync(0xffffffffu, x, o);
+                    if (lane >= o) x += y;
+                }
+                incl = x;
+            }
+            if (s) {
+                const u64 r = base_c + sm.part_count[k * kWarps + warp] + rank;
+                p.survivor_idx[r] = (int32_t)(q0 + (int64_t)k * kThreads + tid);
+                p.cu_seqlens[r + 1] = (int64_t)(base_t + sm.part_tokens[k * kWarps + warp] + incl);
+            }
         }
     }
-    }  // DO_COMPACT
 }
 
-template <int E_T, int CONF, bool DO_GATE, bool DO_COMPACT, int ITEMS>
+// Questions per thread: as many as needed for the grid to be one co-resident wave
+// (kBlocksPerSM blocks per SM), capped by what a block keeps in shared memory.
+inline int choose_items(int64_t Q, int max_items) {
+    const int64_t wave = (int64_t)num_sms() * kBlocksPerSM * kThreads;
+    int64_t items = (Q + wave - 1) / wave;
+    if (items < 1) items = 1;
+    if (items > max_items) items = max_items;
+    return (int)items;
+}
+
+template <int E_T, int CONF, bool DO_GATE, bool DO_COMPACT, int MAXI, int BATCH>
 mosaic_status_t launch(GateArgs& a, size_t ws_bytes, void* workspace, cudaStream_t stream) {
-    constexpr int TILE = kThreads * ITEMS;
-    const unsigned int tiles = (unsigned int)((a.Q + TILE - 1) / TILE);
+    a.items = choose_items(a.Q, MAXI);
+    const int64_t tile = (int64_t)kThreads * a.items;
+    const unsigned int tiles = (unsigned int)((a.Q + tile - 1) / tile);
     a.num_tiles = tiles;
     if constexpr (DO_COMPACT) {
         const size_t need = sizeof(ScanHeader) + (size_t)tiles * sizeof(TileState);
@@ -375,7 +513,8 @@ mosaic_status_t launch(GateArgs& a, size_t ws_bytes, void* workspace, cudaStream
         a.tiles = reinterpret_cast<TileState*>(static_cast<char*>(workspace) + sizeof(ScanHeader));
         MOSAIC_CUDA_TRY(cudaMemsetAsync(workspace, 0, need, stream));
     }
-    gate_compact_kernel<E_T, CONF, DO_GATE, DO_COMPACT, ITEMS><<<tiles, kThreads, 0, stream>>>(a);
+    gate_compact_kernel<E_T, CONF, DO_GATE, DO_COMPACT, MAXI, BATCH>
+        <<<tiles, kThreads, 0, stream>>>(a);
     count_launch();
     MOSAIC_CUDA_TRY(cudaGetLastError());
     return MOSAIC_OK;
@@ -383,16 +522,17 @@ mosaic_status_t launch(GateArgs& a, size_t ws_bytes, void* workspace, cudaStream
 
 template <int CONF, bool DO_COMPACT>
 mosaic_status_t dispatch_gate(GateArgs& a, size_t ws_bytes, void* ws, cudaStream_t s) {
+    constexpr int M = kMaxItems;
     switch (a.E) {
-        case 1: return launch<1, CONF, true, DO_COMPACT, 4>(a, ws_bytes, ws, s);
-        case 2: return launch<2, CONF, true, DO_COMPACT, 4>(a, ws_bytes, ws, s);
-        case 3: return launch<3, CONF, true, DO_COMPACT, 4>(a, ws_bytes, ws, s);
-        case 4: return launch<4, CONF, true, DO_COMPACT, 4>(a, ws_bytes, ws, s);
-        case 5: return launch<5, CONF, true, DO_COMPACT, 4>(a, ws_bytes, ws, s);
-        case 6: return launch<6, CONF, true, DO_COMPACT, 4>(a, ws_bytes, ws, s);
-        case 7: return launch<7, CONF, true, DO_COMPACT, 4>(a, ws_bytes, ws, s);
-        case 8: return launch<8, CONF, true, DO_COMPACT, 4>(a, ws_bytes, ws, s);
-        default: return launch<0, CONF, true, DO_COMPACT, 1>(a, ws_bytes, ws, s);
+        case 1: return launch<1, CONF, true, DO_COMPACT, M, 4>(a, ws_bytes, ws, s);
+        case 2: return launch<2, CONF, true, DO_COMPACT, M, 4>(a, ws_bytes, ws, s);
+        case 3: return launch<3, CONF, true, DO_COMPACT, M, 4>(a, ws_bytes, ws, s);
+        case 4: return launch<4, CONF, true, DO_COMPACT, M, 4>(a, ws_bytes, ws, s);
+        case 5: return launch<5, CONF, true, DO_COMPACT, M, 4>(a, ws_bytes, ws, s);
+        case 6: return launch<6, CONF, true, DO_COMPACT, M, 4>(a, ws_bytes, ws, s);
+        case 7: return launch<7, CONF, true, DO_COMPACT, M, 4>(a, ws_bytes, ws, s);
+        case 8: return launch<8, CONF, true, DO_COMPACT, M, 4>(a, ws_bytes, ws, s);
+        default: return launch<0, CONF, true, DO_COMPACT, kMaxItemsWide, 1>(a, ws_bytes, ws, s);
     }
 }
 
@@ -405,6 +545,11 @@ mosaic_status_t check_gate_args(const int32_t* answers, const float* expert_conf
     if (Q > 0) {
         if (!answers || !aligned16(answers)) return MOSAIC_ERR_INVALID_ARG;
         if (conf_mode == MOSAIC_CONF_WEIGHTED && (!expert_conf || !aligned16(expert_conf)))
+            return MOSAIC_ERR_INVALID_ARG;
+        // 32-byte rows are read with 256-bit loads
+        if (E % 8 == 0 && E <= 8 &&
+            ((reinterpret_cast<uintptr_t>(answers) & 31u) ||
+             (conf_mode == MOSAIC_CONF_WEIGHTED && (reinterpret_cast<uintptr_t>(expert_conf) & 31u))))
             return MOSAIC_ERR_INVALID_ARG;
     }
     return MOSAIC_OK;
@@ -451,7 +596,8 @@ extern "C" mosaic_status_t mosaic_gate(const int32_t* answers, const float* expe
 
 extern "C" size_t mosaic_compact_workspace_bytes(int64_t Q) {
     if (Q < 0) return 0;
-    const size_t tiles = (size_t)((Q + kMinTile - 1) / kMinTile);
+    // worst case: one question per thread (small Q) -> Q / kThreads tiles
+    const size_t tiles = (size_t)((Q + kThreads - 1) / kThreads);
     return sizeof(ScanHeader) + (tiles + 1) * sizeof(TileState);
 }
 
@@ -476,7 +622,7 @@ extern "C" mosaic_status_t mosaic_compact(const uint8_t* bypass, const int32_t* 
     a.n_survivors = n_survivors;
     a.total_tokens = total_tokens;
     a.max_seqlen = max_seqlen;
-    return launch<1, MOSAIC_CONF_VOTE, false, true, 4>(a, workspace_bytes, workspace, s);
+    return launch<1, MOSAIC_CONF_VOTE, false, true, kMaxItems, 4>(a, workspace_bytes, workspace, s);
 }
 
 extern "C" mosaic_status_t mosaic_gate_compact(
