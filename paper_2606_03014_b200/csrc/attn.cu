@@ -8,12 +8,17 @@
 //   One CTA per SM works through (item, q head) pairs.  A q block is two 128-row tiles; for each
 //   128-key tile j the tensor core computes S_t = Q_t K_j^T into tensor memory, a 128-thread
 //   softmax group per tile (one thread per query row) turns S_t into P_t in place (bf16, same
-//   TMEM columns), and O_t += P_t V_j accumulates in tensor memory.  While one tile is in
-//   softmax the tensor core runs the other tile's MMAs.
-//     warp 0      : TMA producer (Q tiles, K/V ring of kSlots 128-key tiles, 128-byte swizzle)
-//     warp 1      : tcgen05.mma issuer (one elected thread)
-//     warp 2      : TMEM allocation / release
-//     warps 4-7   : softmax + epilogue of tile 0        warps 8-11 : ... of tile 1
+//   TMEM columns), and O_t += P_t V_j accumulates in tensor memory.  The two tiles are two
+//   independent streams that share only the K/V ring: each has its own MMA-issuing thread and
+//   its own softmax group, so one tile's MMAs fill the tensor pipe while the other is in
+//   softmax, and a tile that finishes its item first starts the next item without waiting.
+//     warps 0-3   : softmax + epilogue of tile 0        warps 4-7 : ... of tile 1
+//     warp 8      : TMA producer (Q tiles, K/V ring of kSlots 128-key tiles, 128-byte swizzle)
+//     warp 9, 10  : tcgen05.mma issuer of tile 0 / tile 1 (one elected thread each);
+//                   warp 10 also allocates / releases tensor memory
+//   The two issuers take a lock around each group of MMAs so the groups alternate in the tensor
+//   pipe; a quarter of the exponentials is evaluated on the FMA pipe (exp2_poly2), the rest on MUFU.
+//   (MOSAIC_P_HALVES=1 hands P_t to the tensor core in two halves of 64 keys; off by default.)
 //   The running row max is only moved (and O rescaled) when it grows by more than 2^8, so the
 //   rescale of the accumulator is rare; the final 1/l normalisation makes the result exact.
 #include <cuda.h>
@@ -33,11 +38,28 @@ namespace {
 constexpr int BM = 128;       // query rows per tile  (UMMA M)
 constexpr int BN = 128;       // key rows per tile    (UMMA N of S, UMMA K of PV)
 constexpr int BQ = 2 * BM;    // query rows per work item (two tiles)
-constexpr int kSlots = 4;     // K/V ring depth (tiles)
+#ifndef MOSAIC_KV_SLOTS
+#define MOSAIC_KV_SLOTS 5
+#endif
+constexpr int kSlots = MOSAIC_KV_SLOTS;  // K/V ring depth (tiles)
 constexpr int kThreadsAttn = 384;
+// Warp roles.  The softmax groups take the LOW warp ids (TMEM lane quarter = warp % 4) and the
+// single-thread roles the HIGH ones: the warp schedulers favour the highest warp id among the
+// eligible warps, and the MMA issuers are the threads everything else waits for.
+constexpr int kWarpProducer = 8, kWarpMma0 = 9, kWarpMma1 = 10;  // warp 11: idle
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units
+#ifndef MOSAIC_P_HALVES
+#define MOSAIC_P_HALVES 0
+#endif
+#ifndef MOSAIC_POLY_PAIRS
+#define MOSAIC_POLY_PAIRS 1
+#endif
+#ifndef MOSAIC_MMA_LOCK
+#define MOSAIC_MMA_LOCK 1
+#endif
+constexpr int kPolyPairs = MOSAIC_POLY_PAIRS;  // of every 4 element pairs: exp2 on the FMA pipe
 
 // ------------------------------------------------------------------------------- A5: schedule
 struct SchedHeader {
@@ -50,7 +72,7 @@ struct Workspace {
     int* cnt;     // [levels]  sequences with exactly c+1 q blocks -> sequences with more than c
     int* start;   // [levels]  first entry of level c (levels in descending order)
     int* cursor;  // [levels]
-    int2* items;  // [capacity] (sequence, q block)
+    int4* items;  // [capacity] (first token of the sequence, its length, q block, sequence)
     size_t zero_bytes;  // prefix that must be zeroed before schedule_kernel
     size_t total_bytes;
 };
@@ -71,8 +93,8 @@ inline Workspace carve(void* base, int32_t n_seqs, int64_t total_tokens) {
     w.start = reinterpret_cast<int*>(p + off);
     off += levels * sizeof(int);
     off = (off + 15) & ~size_t(15);
-    w.items = reinterpret_cast<int2*>(p + off);
-    off += cap * sizeof(int2);
+    w.items = reinterpret_cast<int4*>(p + off);
+    off += cap * sizeof(int4);
     w.total_bytes = (off + 255) & ~size_t(255);
     return w;
 }
@@ -80,37 +102,65 @@ inline Workspace carve(void* base, int32_t n_seqs, int64_t total_tokens) {
 // Work items in descending cost order.  The cost of (sequence s, q block c) is its number of KV
 // tiles, ~2c + 2, so "longest first" is "descending c": level c holds one entry for every
 // sequence with more than c blocks.  Counting sort over levels; order inside a level is arbitrary
-// (the results do not depend on the schedule).  One block.
+// (the results do not depend on the schedule).  One block; the two scans over the levels are
+// chunked over its threads.
+
+// Sum of v over the threads with a larger thread index (whole block calls).
+__device__ __forceinline__ int block_suffix_exclusive(int v, int* warp_tot /* [32] shared */) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    int x = v;  // inclusive suffix inside the warp
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_down_sync(0xffffffffu, x, o);
+        if (lane + o < 32) x += y;
+    }
+    __syncthreads();  // warp_tot may still be read from a previous call
+    if (lane == 0) warp_tot[warp] = x;
+    __syncthreads();
+    int above = 0;
+    for (int w = warp + 1; w < nwarp; ++w) above += warp_tot[w];
+    return above + x - v;
+}
+
 __global__ void __launch_bounds__(1024) schedule_kernel(const int64_t* __restrict__ cu_seqlens,
                                                         int n_seqs, int levels, SchedHeader* header,
                                                         int* cnt, int* start, int* cursor,
-                                                        int2* items) {
-    for (int s = threadIdx.x; s < n_seqs; s += blockDim.x) {
+                                                        int4* items) {
+    __shared__ int warp_tot[32];
+    const int tid = threadIdx.x;
+    for (int s = tid; s < n_seqs; s += blockDim.x) {
         const int64_t L = cu_seqlens[s + 1] - cu_seqlens[s];
         const int nb = (int)((L + BQ - 1) / BQ);
         if (nb > 0) atomicAdd(&cnt[min(nb, levels) - 1], 1);
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        int run = 0;
-        for (int c = levels - 1; c >= 0; --c) {  // suffix sum: sequences with more than c blocks
-            run += cnt[c];
-            cnt[c] = run;
-        }
-        int pos = 0;
-        for (int c = levels - 1; c >= 0; --c) {
-            start[c] = pos;
-            pos += cnt[c];
-        }
-        header->n_items = pos;
+    const int chunk = (levels + (int)blockDim.x - 1) / (int)blockDim.x;
+    const int lo = min(levels, tid * chunk), hi = min(levels, lo + chunk);
+    // cnt[c] <- number of sequences with more than c blocks (inclusive suffix sum)
+    int local = 0;
+    for (int c = lo; c < hi; ++c) local += cnt[c];
+    int run = block_suffix_exclusive(local, warp_tot);
+    for (int c = hi - 1; c >= lo; --c) {
+        run += cnt[c];
+        cnt[c] = run;
     }
+    // start[c] <- entries of the levels above c (exclusive suffix sum of the new cnt)
+    local = 0;
+    for (int c = lo; c < hi; ++c) local += cnt[c];
+    int pos = block_suffix_exclusive(local, warp_tot);
+    for (int c = hi - 1; c >= lo; --c) {
+        start[c] = pos;
+        pos += cnt[c];
+    }
+    if (tid == 0) header->n_items = pos;  // thread 0 owns level 0: pos = all entries
     __syncthreads();
-    for (int s = threadIdx.x; s < n_seqs; s += blockDim.x) {
+    for (int s = tid; s < n_seqs; s += blockDim.x) {
         const int64_t L = cu_seqlens[s + 1] - cu_seqlens[s];
         const int nb = min((int)((L + BQ - 1) / BQ), levels);
+        const int t0 = (int)cu_seqlens[s];  // total_tokens < 2^31
         for (int c = 0; c < nb; ++c) {
-            const int pos = start[c] + atomicAdd(&cursor[c], 1);
-            items[pos] = make_int2(s, c);
+            const int at = start[c] + atomicAdd(&cursor[c], 1);
+            items[at] = make_int4(t0, (int)L, c, s);  // everything a CTA needs, in one load
         }
     }
 }
@@ -118,13 +168,14 @@ __global__ void __launch_bounds__(1024) schedule_kernel(const int64_t* __restric
 // ------------------------------------------------------------------------------ A1-A4: forward
 struct AttnParams {
     const int64_t* cu_seqlens;
-    const int2* items;
+    const int4* items;
     const SchedHeader* header;
     __nv_bfloat16* o;
     float* lse;
     int64_t T;
     int Hq, Hkv;
     float scale_log2;  // |softmax_scale| * log2(e); a negative scale negates Q inside the MMA
+    int o_align32;     // o is 32-byte aligned: the epilogue may use 256-bit stores
 };
 
 template <int D>
@@ -134,9 +185,24 @@ struct SmemLayout {
     static constexpr int kQ = 0;                    // Q_0, Q_1
     static constexpr int kKV = 2 * kTileBytes;      // ring of kSlots tiles
     static constexpr int kBars = kKV + kSlots * kTileBytes;
-    static constexpr int kTotal = kBars + 256;
+    static constexpr int kTotal = kBars + 512;
     static constexpr int kDynamic = kTotal + 1024;  // slack for the 1024-byte alignment
+    static_assert(kDynamic <= 227 * 1024, "shared memory of one CTA");
 };
+
+// mbarriers (8 bytes each) inside the kBars region
+enum Bar : uint32_t {
+    kBarQFull = 0,                          // [2]  Q_t landed                       (TMA tx)
+    kBarQEmpty = 2,                         // [2]  last S_t of the item has read Q_t (commit)
+    kBarKvFull = 4,                         // [kSlots] K_j / V_j landed             (TMA tx)
+    kBarKvEmpty = 4 + kSlots,               // [2][kSlots] stream t is done with the slot
+    kBarSFull = 4 + 3 * kSlots,             // [2]  S_t complete                     (commit)
+    kBarPHalf = kBarSFull + 2,              // [2]  keys 0-63 of P_t written         (4 warps)
+    kBarPFull = kBarSFull + 4,              // [2]  keys 64-127 of P_t written       (4 warps)
+    kBarODone = kBarSFull + 6,              // [2]  last PV_t of the item complete   (commit)
+    kNumBars = kBarSFull + 8
+};
+static_assert(kNumBars * 8 + 8 <= 512, "barrier region");
 
 // One (work item, q head) pair as every warp role sees it.
 struct Work {
@@ -153,12 +219,12 @@ __device__ __forceinline__ Work decode_work(const AttnParams& p, int w) {
     const int item = w / p.Hq;
     k.h = w - item * p.Hq;
     k.g = k.h / (p.Hq / p.Hkv);
-    const int2 it = p.items[item];
-    k.t0 = p.cu_seqlens[it.x];
-    k.L = (int)(p.cu_seqlens[it.x + 1] - k.t0);
-    k.row0 = it.y * BQ;
-    k.n[0] = 2 * it.y + 1;
-    k.n[1] = (k.row0 + BM < k.L) ? 2 * it.y + 2 : 0;
+    const int4 it = __ldg(p.items + item);
+    k.t0 = it.x;
+    k.L = it.y;
+    k.row0 = it.z * BQ;
+    k.n[0] = 2 * it.z + 1;
+    k.n[1] = (k.row0 + BM < k.L) ? 2 * it.z + 2 : 0;
     k.n_kv = max(k.n[0], k.n[1]);
     return k;
 }
@@ -167,6 +233,23 @@ __device__ __forceinline__ float ex2_approx(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
+}
+// 2^x for two x <= ~100 on the FMA pipe: x = n + f with n = round(x) taken from the low mantissa
+// bits of x + 1.5 * 2^23, 2^f on [-0.5, 0.5] by a degree-3 minimax polynomial (relative error
+// 7.5e-5, far below the 2^-9 rounding of P to bf16), 2^n added into the exponent field.
+__device__ __forceinline__ float2 exp2_poly2(float2 x) {
+    x.x = fmaxf(x.x, -126.f);
+    x.y = fmaxf(x.y, -126.f);
+    const float2 t = __fadd2_rn(x, make_float2(12582912.f, 12582912.f));
+    const float2 n = __fadd2_rn(t, make_float2(-12582912.f, -12582912.f));
+    const float2 f = __ffma2_rn(n, make_float2(-1.f, -1.f), x);
+    float2 p = __ffma2_rn(make_float2(0.055172015f, 0.055172015f), f,
+                          make_float2(0.24261113f, 0.24261113f));
+    p = __ffma2_rn(p, f, make_float2(0.69326091f, 0.69326091f));
+    p = __ffma2_rn(p, f, make_float2(0.99992806f, 0.99992806f));
+    p.x = __int_as_float(__float_as_int(p.x) + (__float_as_int(t.x) << 23));
+    p.y = __int_as_float(__float_as_int(p.y) + (__float_as_int(t.y) << 23));
+    return p;
 }
 template <int N>
 __device__ __forceinline__ void setmaxnreg_inc() {
@@ -189,13 +272,11 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
     uint8_t* smem = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
     const uint32_t sQ = smem_base + SL::kQ, sKV = smem_base + SL::kKV;
     const uint32_t bars = smem_base + SL::kBars;
-    const uint32_t bar_q_full = bars, bar_q_empty = bars + 8;
-    auto bar_kv_full = [&](int s) { return bars + 16 + 8 * s; };
-    auto bar_kv_empty = [&](int s) { return bars + 16 + 8 * kSlots + 8 * s; };
-    auto bar_s_full = [&](int t) { return bars + 16 + 16 * kSlots + 8 * t; };
-    auto bar_p_full = [&](int t) { return bars + 32 + 16 * kSlots + 8 * t; };
-    auto bar_o_done = [&](int t) { return bars + 48 + 16 * kSlots + 8 * t; };
-    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + SL::kBars + 192);
+    auto bar = [&](uint32_t which, int i = 0) { return bars + 8u * (which + (uint32_t)i); };
+    auto bar_kv_empty = [&](int t, uint32_t slot) { return bar(kBarKvEmpty, t * kSlots + (int)slot); };
+    volatile uint32_t* tmem_slot =
+        reinterpret_cast<volatile uint32_t*>(smem + SL::kBars + 8 * kNumBars);
+    const uint32_t mma_lock = bars + 8 * kNumBars + 4;  // the two issuers take turns (see below)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int n_work = p.header->n_items * p.Hq;
@@ -204,20 +285,20 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         ptx::prefetch_tensormap(&tm_q);
         ptx::prefetch_tensormap(&tm_k);
         ptx::prefetch_tensormap(&tm_v);
-        ptx::mbar_init(bar_q_full, 1);
-        ptx::mbar_init(bar_q_empty, 1);
-        for (int s = 0; s < kSlots; ++s) {
-            ptx::mbar_init(bar_kv_full(s), 1);
-            ptx::mbar_init(bar_kv_empty(s), 1);
-        }
         for (int t = 0; t < 2; ++t) {
-            ptx::mbar_init(bar_s_full(t), 1);
-            ptx::mbar_init(bar_p_full(t), BM);
-            ptx::mbar_init(bar_o_done(t), 1);
+            ptx::mbar_init(bar(kBarQFull, t), 1);
+            ptx::mbar_init(bar(kBarQEmpty, t), 1);
+            ptx::mbar_init(bar(kBarSFull, t), 1);
+            ptx::mbar_init(bar(kBarPHalf, t), BM / 32);
+            ptx::mbar_init(bar(kBarPFull, t), BM / 32);
+            ptx::mbar_init(bar(kBarODone, t), 1);
+            for (int s = 0; s < kSlots; ++s) ptx::mbar_init(bar_kv_empty(t, s), 1);
         }
+        for (int s = 0; s < kSlots; ++s) ptx::mbar_init(bar(kBarKvFull, s), 1);
+        asm volatile("st.shared.u32 [%0], %1;" ::"r"(mma_lock), "r"(0u) : "memory");
         ptx::fence_barrier_init();
     }
-    if (warp == 2) {
+    if (warp == kWarpMma1) {
         ptx::tmem_alloc<kTmemCols>(ptx::smem_u32(const_cast<uint32_t*>(tmem_slot)));
         ptx::tmem_relinquish();
     }
@@ -226,129 +307,199 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
 
-    if (warp < 4) {
+    // Position q of the K/V ring sequence (K_0, V_0, K_1, V_1, ... of one item after the other)
+    // lives in slot q % kSlots; its full / empty barriers are in phase (q / kSlots) & 1.
+    auto slot_of = [](uint32_t q) { return q % kSlots; };
+    auto phase_of = [](uint32_t q) { return (q / kSlots) & 1u; };
+
+    if (warp >= 8) {
         setmaxnreg_dec<80>();
-        if (warp == 0 && lane == 0) {
+        if (warp == kWarpProducer) {
             // ================================ TMA producer ================================
-            int slot = 0;
-            uint32_t ph_kv = 0, ph_q = 0;
+            uint32_t pos = 0, ph_q[2] = {0, 0};
+            Work next_k{};
+            if ((int)blockIdx.x < n_work) next_k = decode_work(p, blockIdx.x);
             for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-                const Work k = decode_work(p, w);
-                ptx::mbar_wait(bar_q_empty, ph_q ^ 1);
-                ph_q ^= 1;
-                const int nq = k.n[1] ? 2 : 1;
-                ptx::mbar_arrive_expect_tx(bar_q_full, nq * SL::kTileBytes);
-                for (int t = 0; t < nq; ++t)
-#pragma unroll
-                    for (int c = 0; c < D / 64; ++c)
-                        ptx::tma_load_3d(sQ + t * SL::kTileBytes + c * SL::kBlockBytes, &tm_q,
-                                         bar_q_full, c * 64, k.h, (int)(k.t0 + k.row0 + t * BM));
-                for (int j = 0; j < k.n_kv; ++j) {
-#pragma unroll
-                    for (int kv = 0; kv < 2; ++kv) {  // K_j then V_j
-                        ptx::mbar_wait(bar_kv_empty(slot), ph_kv ^ 1);
-                        ptx::mbar_arrive_expect_tx(bar_kv_full(slot), SL::kTileBytes);
+                const Work k = next_k;  // the next item is decoded one item ahead (L2 latency)
+                if (w + (int)gridDim.x < n_work) next_k = decode_work(p, w + gridDim.x);
+                auto load_q = [&](int t) {
+                    ptx::mbar_wait(bar(kBarQEmpty, t), ph_q[t] ^ 1);
+                    ph_q[t] ^= 1;
+                    if (ptx::elect_one()) {
+                        ptx::mbar_arrive_expect_tx(bar(kBarQFull, t), SL::kTileBytes);
 #pragma unroll
                         for (int c = 0; c < D / 64; ++c)
-                            ptx::tma_load_3d(sKV + slot * SL::kTileBytes + c * SL::kBlockBytes,
-                                             kv == 0 ? &tm_k : &tm_v, bar_kv_full(slot), c * 64,
-                                             k.g, (int)(k.t0 + j * BN));
-                        if (++slot == kSlots) {
-                            slot = 0;
-                            ph_kv ^= 1;
-                        }
+                            ptx::tma_load_3d(sQ + t * SL::kTileBytes + c * SL::kBlockBytes, &tm_q,
+                                             bar(kBarQFull, t), c * 64, k.h,
+                                             (int)(k.t0 + k.row0 + t * BM));
                     }
+                    __syncwarp();
+                };
+                auto load_kv = [&](const CUtensorMap* tm, int j) {
+                    const uint32_t slot = slot_of(pos), ph = phase_of(pos);
+                    ++pos;
+                    ptx::mbar_wait(bar_kv_empty(0, slot), ph ^ 1);
+                    ptx::mbar_wait(bar_kv_empty(1, slot), ph ^ 1);
+                    if (ptx::elect_one()) {
+                        ptx::mbar_arrive_expect_tx(bar(kBarKvFull, slot), SL::kTileBytes);
+#pragma unroll
+                        for (int c = 0; c < D / 64; ++c)
+                            ptx::tma_load_3d(sKV + slot * SL::kTileBytes + c * SL::kBlockBytes, tm,
+                                             bar(kBarKvFull, slot), c * 64, k.g,
+                                             (int)(k.t0 + j * BN));
+                    }
+                    __syncwarp();
+                };
+                load_q(0);
+                load_kv(&tm_k, 0);
+                if (k.n[1]) load_q(1);
+                load_kv(&tm_v, 0);
+                for (int j = 1; j < k.n_kv; ++j) {
+                    load_kv(&tm_k, j);
+                    load_kv(&tm_v, j);
                 }
             }
-        } else if (warp == 1 && lane == 0) {
-            // ================================ MMA issuer ==================================
+        } else if (warp == kWarpMma0 || warp == kWarpMma1) {
+            // ===================== MMA issuer of tile t = warp - kWarpMma0 =====================
+            const int t = warp - kWarpMma0;
             const uint32_t idesc_s =
                 ptx::umma_idesc_bf16(BM, BN, false, false) | (negate_q ? (1u << 13) : 0u);
             constexpr uint32_t idesc_pv = ptx::umma_idesc_bf16(BM, D, false, true);
-            int slot = 0;
-            uint32_t ph_kv = 0, ph_q = 0, ph_p[2] = {0, 0};
-            auto advance = [&]() {
-                if (++slot == kSlots) {
-                    slot = 0;
-                    ph_kv ^= 1;
-                }
-            };
+            const uint32_t tS = tmem + t * 128, tO = tmem + 256 + t * 128;
+            const uint32_t q_smem = sQ + t * SL::kTileBytes;
+            auto kv_wait = [&](uint32_t q) { ptx::mbar_wait(bar(kBarKvFull, slot_of(q)), phase_of(q)); };
             // S_t = Q_t K^T : both operands K-major (D contiguous), 128-byte swizzle
-            auto issue_qk = [&](int t, int kslot) {
-                const uint32_t a = sQ + t * SL::kTileBytes, b = sKV + kslot * SL::kTileBytes;
+            // (descriptors of the k-th 16-wide slice = descriptor of the tile + a constant in the
+            //  14-bit start-address field; tiles are 1024-byte aligned and < 256 KB, so no carry)
+            const uint64_t q_desc = ptx::umma_smem_desc_sw128(q_smem, 16, 1024);
+            auto issue_qk = [&](uint32_t kslot) {
+                const uint64_t k_desc = ptx::umma_smem_desc_sw128(sKV + kslot * SL::kTileBytes, 16, 1024);
 #pragma unroll
                 for (int kk = 0; kk < D / 16; ++kk) {
-                    const uint32_t off = (kk / 4) * SL::kBlockBytes + (kk % 4) * 32;
-                    ptx::umma_ss(tmem + t * 128, ptx::umma_smem_desc_sw128(a + off, 16, 1024),
-                                 ptx::umma_smem_desc_sw128(b + off, 16, 1024), idesc_s, kk > 0);
+                    constexpr int kBlk = SL::kBlockBytes;
+                    const uint64_t off = (uint64_t)(((kk / 4) * kBlk + (kk % 4) * 32) >> 4);
+                    ptx::umma_ss(tS, q_desc + off, k_desc + off, idesc_s, kk > 0);
                 }
-                ptx::umma_commit(bar_s_full(t));
             };
-            // O_t (+)= P_t V : A = P_t from tensor memory, B = V (MN-major: D contiguous)
-            auto issue_pv = [&](int t, int vslot, bool accumulate) {
-                const uint32_t b = sKV + vslot * SL::kTileBytes;
+            // O_t (+)= P_t[:, 16 kk0 .. 16 kk1) V : A = P_t from tensor memory, B = V (MN-major)
+            auto issue_pv = [&](uint32_t vslot, int kk0, int kk1, bool accumulate) {
+                const uint64_t v_desc =
+                    ptx::umma_smem_desc_sw128(sKV + vslot * SL::kTileBytes, SL::kBlockBytes, 1024);
 #pragma unroll
-                for (int kk = 0; kk < BN / 16; ++kk)
-                    ptx::umma_ts(tmem + 256 + t * 128, tmem + t * 128 + kk * 8,
-                                 ptx::umma_smem_desc_sw128(b + kk * 2048, SL::kBlockBytes, 1024),
-                                 idesc_pv, (accumulate || kk > 0) ? 1u : 0u);
+                for (int kk = kk0; kk < kk1; ++kk)
+                    ptx::umma_ts(tO, tS + kk * 8, v_desc + (uint64_t)((kk * 2048) >> 4), idesc_pv,
+                                 (accumulate || kk > kk0) ? 1u : 0u);
             };
+            // The tensor pipe runs MMAs in issue order.  Each issuer holds this lock while it
+            // issues one group of MMAs, so the groups of the two tiles alternate instead of
+            // interleaving instruction by instruction: their S tiles then complete half a step
+            // apart and the two softmax groups stay out of phase.
+            auto lock = [&]() {
+#if MOSAIC_MMA_LOCK
+                uint32_t old;
+                do {
+                    asm volatile("atom.shared.relaxed.cta.cas.b32 %0, [%1], 0, 1;"
+                                 : "=r"(old) : "r"(mma_lock) : "memory");
+                } while (old != 0);
+#endif
+            };
+            auto unlock = [&]() {
+#if MOSAIC_MMA_LOCK
+                asm volatile("st.shared.relaxed.cta.u32 [%0], %1;" ::"r"(mma_lock), "r"(0u) : "memory");
+#endif
+            };
+            // The whole warp walks the work list (uniform control flow keeps the descriptors in
+            // uniform registers); one elected lane issues the MMAs and their commits.
+            uint32_t pos = 0, ph_q = 0, ph_p = 0;
+            Work next_k{};
+            if ((int)blockIdx.x < n_work) next_k = decode_work(p, blockIdx.x);
             for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-                const Work k = decode_work(p, w);
-                ptx::mbar_wait(bar_q_full, ph_q);
-                ph_q ^= 1;
-                ptx::mbar_wait(bar_kv_full(slot), ph_kv);  // K_0
-                ptx::tc_fence_after();
-                issue_qk(0, slot);
-                if (k.n[1]) issue_qk(1, slot);
-                ptx::umma_commit(bar_kv_empty(slot));
-                advance();
-                for (int j = 0; j < k.n_kv; ++j) {
-                    const int vslot = slot;
-                    const uint32_t vph = ph_kv;
-                    advance();
-                    const int kslot = slot;  // K_{j+1}, if any
-                    const bool has_next = j + 1 < k.n_kv;
-                    ptx::mbar_wait(bar_kv_full(vslot), vph);
-                    if (has_next) ptx::mbar_wait(bar_kv_full(kslot), ph_kv);
-#pragma unroll
-                    for (int t = 0; t < 2; ++t) {
-                        if (j < k.n[t]) {
-                            ptx::mbar_wait(bar_p_full(t), ph_p[t]);
-                            ph_p[t] ^= 1;
-                            ptx::tc_fence_after();
-                            issue_pv(t, vslot, j > 0);
-                            if (j + 1 < k.n[t]) issue_qk(t, kslot);
-                            if (j == k.n[t] - 1) ptx::umma_commit(bar_o_done(t));
-                        }
+                const Work k = next_k;  // the next item is decoded one item ahead (L2 latency)
+                if (w + (int)gridDim.x < n_work) next_k = decode_work(p, w + gridDim.x);
+                const int n_t = k.n[t];
+                const uint32_t base = pos;
+                if (n_t > 0) {
+                    ptx::mbar_wait(bar(kBarQFull, t), ph_q);
+                    ph_q ^= 1;
+                    kv_wait(base);  // K_0
+                    ptx::tc_fence_after();
+                    if (ptx::elect_one()) {
+                        lock();
+                        issue_qk(slot_of(base));
+                        ptx::umma_commit(bar(kBarSFull, t));
+                        ptx::umma_commit(bar_kv_empty(t, slot_of(base)));
+                        if (n_t == 1) ptx::umma_commit(bar(kBarQEmpty, t));
+                        unlock();
                     }
-                    ptx::umma_commit(bar_kv_empty(vslot));
-                    if (has_next) {
-                        ptx::umma_commit(bar_kv_empty(kslot));
-                        advance();
+                    __syncwarp();
+                    for (int j = 0; j < n_t; ++j) {
+                        const uint32_t vpos = base + 2 * j + 1, kpos = vpos + 1;  // V_j, K_{j+1}
+                        const bool more = j + 1 < n_t;
+                        kv_wait(vpos);
+#if MOSAIC_P_HALVES
+                        ptx::mbar_wait(bar(kBarPHalf, t), ph_p);
+                        ptx::tc_fence_after();
+                        if (ptx::elect_one()) {
+                            lock();
+                            issue_pv(slot_of(vpos), 0, BN / 32, j > 0);
+                            unlock();
+                        }
+                        __syncwarp();
+#endif
+                        if (more) kv_wait(kpos);
+                        ptx::mbar_wait(bar(kBarPFull, t), ph_p);
+                        ph_p ^= 1;
+                        ptx::tc_fence_after();
+                        if (ptx::elect_one()) {
+                            lock();
+                            if (MOSAIC_P_HALVES)
+                                issue_pv(slot_of(vpos), BN / 32, BN / 16, true);
+                            else
+                                issue_pv(slot_of(vpos), 0, BN / 16, j > 0);
+                            ptx::umma_commit(bar_kv_empty(t, slot_of(vpos)));
+                            if (more) {
+                                issue_qk(slot_of(kpos));
+                                ptx::umma_commit(bar(kBarSFull, t));
+                                ptx::umma_commit(bar_kv_empty(t, slot_of(kpos)));
+                                if (j + 2 == n_t) ptx::umma_commit(bar(kBarQEmpty, t));
+                            } else {
+                                ptx::umma_commit(bar(kBarODone, t));
+                            }
+                            unlock();
+                        }
+                        __syncwarp();
                     }
                 }
-                ptx::umma_commit(bar_q_empty);
+                // ring positions of this item that tile t does not use: consume and release
+                pos = base + 2 * k.n_kv;
+                for (uint32_t q = base + 2 * n_t; q < pos; ++q) {
+                    kv_wait(q);
+                    if (ptx::elect_one()) ptx::mbar_arrive(bar_kv_empty(t, slot_of(q)));
+                    __syncwarp();
+                }
             }
         }
     } else {
         // ============================ softmax + epilogue groups ===========================
         setmaxnreg_inc<208>();
-        const int t = (warp >> 2) - 1;             // tile of this group (0 or 1)
-        const int row = tid - (t + 1) * BM;        // query row inside the tile == TMEM lane
+        const int t = warp >> 2;                   // tile of this group (0 or 1)
+        const int row = tid - t * BM;              // query row inside the tile == TMEM lane
         const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
         const uint32_t tS = tmem + t * 128 + lane_off;        // S_t, overwritten by P_t (bf16)
         const uint32_t tO = tmem + 256 + t * 128 + lane_off;  // O_t
         const float sc = p.scale_log2;
         uint32_t ph_s = 0, ph_o = 0;
 
+        Work next_k{};
+            if ((int)blockIdx.x < n_work) next_k = decode_work(p, blockIdx.x);
         for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-            const Work k = decode_work(p, w);
+            const Work k = next_k;  // the next item is decoded one item ahead (L2 latency)
+            if (w + (int)gridDim.x < n_work) next_k = decode_work(p, w + gridDim.x);
             const int n_t = k.n[t];
             if (n_t == 0) continue;  // this tile has no rows in this block
             float m_used = 0.f, l_run = 0.f;
             for (int j = 0; j < n_t; ++j) {
-                ptx::mbar_wait(bar_s_full(t), ph_s);
+                ptx::mbar_wait(bar(kBarSFull, t), ph_s);
                 ph_s ^= 1;
                 ptx::tc_fence_after();
                 // ---- A2: scores of this row, running max -------------------------------------
@@ -394,46 +545,60 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                     }
                 }
                 // ---- P = exp2(s * scale_log2 - m), row sum, bf16 pairs into the S columns ------
-                float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
-                auto exp_pass = [&](auto is_diag) {
+                // Two elements at a time (packed fp32 FMA / ADD).  Of every four pairs, kPolyPairs
+                // are exponentiated on the FMA pipe (exp2_poly2) and the rest on the MUFU unit, whose
+                // 16 results per clock per SM would otherwise bound the whole kernel.
+                float2 la = make_float2(0.f, 0.f), lb = make_float2(0.f, 0.f);
+                const float2 sc2 = make_float2(sc, sc), nm2 = make_float2(-m_used, -m_used);
+                auto exp_half = [&](auto is_diag, int c0) {
                     constexpr bool kDiag = decltype(is_diag)::value;
-                    auto arg = [&](float x) {
-                        const float a = fmaf(x, sc, -m_used);
-                        // a masked key must give exactly 0 even when scale_log2 == 0 (-inf * 0)
-                        return (kDiag && x == -INFINITY) ? -INFINITY : a;
-                    };
 #pragma unroll
-                    for (int c = 0; c < BN / 32; ++c) {
+                    for (int c = c0; c < c0 + BN / 64; ++c) {
                         uint32_t pk[16];
 #pragma unroll
-                        for (int i = 0; i < 32; i += 4) {
-                            const float p0 = ex2_approx(arg(s[c * 32 + i + 0]));
-                            const float p1 = ex2_approx(arg(s[c * 32 + i + 1]));
-                            const float p2 = ex2_approx(arg(s[c * 32 + i + 2]));
-                            const float p3 = ex2_approx(arg(s[c * 32 + i + 3]));
-                            l0 += p0;
-                            l1 += p1;
-                            l2 += p2;
-                            l3 += p3;
-                            __nv_bfloat162 h0 = __floats2bfloat162_rn(p0, p1);
-                            __nv_bfloat162 h1 = __floats2bfloat162_rn(p2, p3);
-                            pk[i / 2] = *reinterpret_cast<uint32_t*>(&h0);
-                            pk[i / 2 + 1] = *reinterpret_cast<uint32_t*>(&h1);
+                        for (int i = 0; i < 32; i += 2) {
+                            const float x0 = s[c * 32 + i], x1 = s[c * 32 + i + 1];
+                            float2 e;
+                            if constexpr (kDiag) {
+                                // a masked key must give exactly 0 even when scale_log2 == 0 (-inf * 0)
+                                const float a0 = fmaf(x0, sc, -m_used), a1 = fmaf(x1, sc, -m_used);
+                                e.x = ex2_approx(x0 == -INFINITY ? -INFINITY : a0);
+                                e.y = ex2_approx(x1 == -INFINITY ? -INFINITY : a1);
+                            } else {
+                                const float2 a = __ffma2_rn(make_float2(x0, x1), sc2, nm2);
+                                if (((i >> 1) & 3) < kPolyPairs)
+                                    e = exp2_poly2(a);
+                                else
+                                    e = make_float2(ex2_approx(a.x), ex2_approx(a.y));
+                            }
+                            if ((i >> 1) & 1)
+                                lb = __fadd2_rn(lb, e);
+                            else
+                                la = __fadd2_rn(la, e);
+                            __nv_bfloat162 h = __floats2bfloat162_rn(e.x, e.y);
+                            pk[i / 2] = *reinterpret_cast<uint32_t*>(&h);
                         }
                         ptx::tmem_st16(tS + c * 16, pk);
                     }
+                    // this half of P_t is in tensor memory: hand it to the MMA issuer
+                    if (MOSAIC_P_HALVES || c0 != 0) {
+                        ptx::tmem_wait_st();
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive(bar(c0 == 0 ? kBarPHalf : kBarPFull, t));
+                    }
                 };
-                if (diag)
-                    exp_pass(std::true_type{});
-                else
-                    exp_pass(std::false_type{});
-                l_run += (l0 + l1) + (l2 + l3);
-                ptx::tmem_wait_st();
-                ptx::tc_fence_before();
-                ptx::mbar_arrive(bar_p_full(t));
+                if (diag) {
+                    exp_half(std::true_type{}, 0);
+                    exp_half(std::true_type{}, BN / 64);
+                } else {
+                    exp_half(std::false_type{}, 0);
+                    exp_half(std::false_type{}, BN / 64);
+                }
+                l_run += (la.x + la.y) + (lb.x + lb.y);
             }
             // ---- epilogue: O_t / l -> bf16 -> global; A4: logsumexp ---------------------------------
-            ptx::mbar_wait(bar_o_done(t), ph_o);
+            ptx::mbar_wait(bar(kBarODone, t), ph_o);
             ph_o ^= 1;
             ptx::tc_fence_after();
             const int row_g = k.row0 + t * BM + row;
@@ -445,22 +610,27 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                 ptx::tmem_ld32(tO + c * 32, r);
                 ptx::tmem_wait_ld();
                 if (row_g < k.L) {
+                    uint32_t pk[16];
 #pragma unroll
-                    for (int i = 0; i < 32; i += 8) {
-                        uint4 v;
-                        __nv_bfloat162 h0 = __floats2bfloat162_rn(__uint_as_float(r[i + 0]) * inv_l,
-                                                                  __uint_as_float(r[i + 1]) * inv_l);
-                        __nv_bfloat162 h1 = __floats2bfloat162_rn(__uint_as_float(r[i + 2]) * inv_l,
-                                                                  __uint_as_float(r[i + 3]) * inv_l);
-                        __nv_bfloat162 h2 = __floats2bfloat162_rn(__uint_as_float(r[i + 4]) * inv_l,
-                                                                  __uint_as_float(r[i + 5]) * inv_l);
-                        __nv_bfloat162 h3 = __floats2bfloat162_rn(__uint_as_float(r[i + 6]) * inv_l,
-                                                                  __uint_as_float(r[i + 7]) * inv_l);
-                        v.x = *reinterpret_cast<uint32_t*>(&h0);
-                        v.y = *reinterpret_cast<uint32_t*>(&h1);
-                        v.z = *reinterpret_cast<uint32_t*>(&h2);
-                        v.w = *reinterpret_cast<uint32_t*>(&h3);
-                        *reinterpret_cast<uint4*>(orow + c * 32 + i) = v;
+                    for (int i = 0; i < 32; i += 2) {
+                        __nv_bfloat162 h = __floats2bfloat162_rn(__uint_as_float(r[i]) * inv_l,
+                                                                 __uint_as_float(r[i + 1]) * inv_l);
+                        pk[i / 2] = *reinterpret_cast<uint32_t*>(&h);
+                    }
+                    // one full 32-byte sector per store when the row is 32-byte aligned
+                    if (p.o_align32) {
+#pragma unroll
+                        for (int i = 0; i < 16; i += 8)
+                            asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(
+                                             orow + c * 32 + 2 * i),
+                                         "r"(pk[i]), "r"(pk[i + 1]), "r"(pk[i + 2]), "r"(pk[i + 3]),
+                                         "r"(pk[i + 4]), "r"(pk[i + 5]), "r"(pk[i + 6]), "r"(pk[i + 7])
+                                         : "memory");
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 16; i += 4)
+                            *reinterpret_cast<uint4*>(orow + c * 32 + 2 * i) =
+                                make_uint4(pk[i], pk[i + 1], pk[i + 2], pk[i + 3]);
                     }
                 }
             }
@@ -472,7 +642,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
 
     ptx::tc_fence_before();
     __syncthreads();
-    if (warp == 2) ptx::tmem_dealloc<kTmemCols>(tmem);
+    if (warp == kWarpMma1) ptx::tmem_dealloc<kTmemCols>(tmem);
 }
 
 // ------------------------------------------------------------------------------------ host side
@@ -581,6 +751,7 @@ extern "C" mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k,
     p.Hq = Hq;
     p.Hkv = Hkv;
     p.scale_log2 = fabsf(softmax_scale) * kLog2e;
+    p.o_align32 = (reinterpret_cast<uintptr_t>(o) & 31u) == 0 ? 1 : 0;
     const int negate_q = softmax_scale < 0.f ? 1 : 0;
     const int64_t max_work = (total_tokens / BQ + n_seqs) * (int64_t)Hq;
     if (max_work >= (1ll << 31)) return MOSAIC_ERR_UNSUPPORTED;
