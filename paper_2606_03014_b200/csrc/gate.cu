@@ -23,11 +23,14 @@
 namespace mosaic {
 namespace {
 
-constexpr int kThreads = 256;
+#ifndef MOSAIC_GATE_THREADS
+#define MOSAIC_GATE_THREADS 256
+#endif
+constexpr int kThreads = MOSAIC_GATE_THREADS;
 constexpr int kWarps = kThreads / 32;
 constexpr int kMaxItems = 16;     // questions per thread, specialised E (<= 8)
 constexpr int kMaxItemsWide = 4;  // ... generic E (<= 32): rows live in 2 x 32 registers
-constexpr int kBlocksPerSM = 2;
+constexpr int kBlocksPerSM = 512 / kThreads;
 
 using u64 = unsigned long long;
 
@@ -160,7 +163,8 @@ __device__ __forceinline__ void sort_labels(int32_t (&s)[N]) {
 template <int EM, int CONF, bool SORTED>
 __device__ __forceinline__ void gate_row(const int32_t (&a)[EM], const float (&w)[EM], int E,
                                          float tau, int32_t& mode, int32_t& count, float& agree,
-                                         float& conf, bool& bypass) {
+                                         float& conf, bool& bypass,
+                                         const float* agree_lut = nullptr) {
     int32_t c_star = 0, md = 0;
     if constexpr (SORTED) {
         int32_t s[EM];
@@ -193,7 +197,8 @@ __device__ __forceinline__ void gate_row(const int32_t (&a)[EM], const float (&w
             }
         }
     }
-    agree = __fdiv_rn((float)c_star, (float)E);
+    // agree_lut[c] holds the same IEEE division, done once per block
+    agree = agree_lut ? agree_lut[c_star] : __fdiv_rn((float)c_star, (float)E);
     conf = agree;
     if constexpr (CONF == MOSAIC_CONF_WEIGHTED) {
         double sm = 0.0, st = 0.0;
@@ -250,18 +255,27 @@ __device__ __forceinline__ Partial look_back(const TileState* tiles, int tile, i
 #pragma unroll
         for (int j = 0; j < W; ++j) {
             const int idx = base - (lane * W + j);
-            lo[j] = hi[j] = kPrefix;  // "tile -1": prefix of nothing
-            if (idx >= 0) ld_state(tiles + idx, lo[j], hi[j]);
+            lo[j] = hi[j] = idx >= 0 ? 0ull : kPrefix;  // "tile -1": prefix of nothing
         }
+        // (re)load every entry that is not published yet, all of them in flight together: one
+        // L2 round trip per pass, however many entries were late
+        bool pending;
+        do {
+#pragma unroll
+            for (int j = 0; j < W; ++j) {
+                const int idx = base - (lane * W + j);
+                const bool ready = (lo[j] >> 62) != 0 && (lo[j] >> 62) == (hi[j] >> 62);
+                if (!ready) ld_state(tiles + idx, lo[j], hi[j]);
+            }
+            pending = false;
+#pragma unroll
+            for (int j = 0; j < W; ++j)
+                pending |= (lo[j] >> 62) == 0 || (lo[j] >> 62) != (hi[j] >> 62);
+        } while (__any_sync(0xffffffffu, pending));
         Partial mine{0, 0, 0};
         bool met = false;
 #pragma unroll
         for (int j = 0; j < W; ++j) {
-            const int idx = base - (lane * W + j);
-            if (idx >= 0) {
-                while ((lo[j] >> 62) == 0 || (lo[j] >> 62) != (hi[j] >> 62))
-                    ld_state(tiles + idx, lo[j], hi[j]);
-            }
             if (!met) {
                 mine.count += lo[j] & kMask31;
                 mine.tokens += hi[j] & kMask62;
@@ -298,6 +312,140 @@ struct GateSmem {
     int warp_max[kWarps];
     unsigned int tile;
 };
+
+// G4-G5 for one tile, after every thread has recorded (survived ? ctx_len : -1) for its questions
+// in sm.len (striped: question = q0 + item * kThreads + thread) and the per-(item, warp) partials:
+// block scan, one look-back round for the tile's exclusive prefix, stable scatter of the survivors.
+template <int MAXI>
+__device__ __forceinline__ void compact_tile(const GateArgs& p, GateSmem<MAXI>& sm, unsigned int tile,
+                                             int64_t q0, int items, int my_max) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // ---- G4-G5: stable compaction and cu_seqlens -------------------------------------------
+    // Scan order inside the tile is (item, thread): exactly ascending question index.
+    my_max = __reduce_max_sync(0xffffffffu, my_max);
+    if (lane == 0) sm.warp_max[warp] = my_max;
+    __syncthreads();
+
+    // (the last warp: the warp scheduler favours the highest warp id, and this warp is what the
+    //  whole tile -- and every later tile -- waits for)
+    if (warp == kWarps - 1) {
+        // exclusive scan of the items * kWarps (<= 128) partials, 4 consecutive per lane
+        constexpr int PER = (MAXI * kWarps + 31) / 32;
+        const int n_part = items * kWarps;
+        unsigned int c[PER];
+        u64 t[PER];
+        unsigned int csum = 0;
+        u64 tsum = 0;
+#pragma unroll
+        for (int j = 0; j < PER; ++j) {
+            const int e = lane * PER + j;
+            c[j] = e < n_part ? sm.part_count[e] : 0u;
+            t[j] = e < n_part ? sm.part_tokens[e] : 0ull;
+            csum += c[j];
+            tsum += t[j];
+        }
+        unsigned int ci = csum;
+        u64 ti = tsum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned int cc = __shfl_up_sync(0xffffffffu, ci, o);
+            const u64 tt = __shfl_up_sync(0xffffffffu, ti, o);
+            if (lane >= o) {
+                ci += cc;
+                ti += tt;
+            }
+        }
+        unsigned int cx = ci - csum;
+        u64 tx = ti - tsum;
+#pragma unroll
+        for (int j = 0; j < PER; ++j) {
+            const int e = lane * PER + j;
+            if (e < n_part) {
+                sm.part_count[e] = cx;
+                sm.part_tokens[e] = tx;
+            }
+            cx += c[j];
+            tx += t[j];
+        }
+        Partial mine;
+        mine.count = __shfl_sync(0xffffffffu, ci, 31);
+        mine.tokens = __shfl_sync(0xffffffffu, ti, 31);
+        mine.max_len = __reduce_max_sync(0xffffffffu, lane < kWarps ? sm.warp_max[lane] : 0);
+
+        TileState* me = p.tiles + tile;
+        Partial before{0, 0, 0};
+        if (tile != 0) {
+            if (lane == 0) st_state(me, pack_lo(kAggregate, mine), kAggregate | mine.tokens);
+            before = look_back(p.tiles, (int)tile, lane);
+        }
+        Partial incl{before.count + mine.count, before.tokens + mine.tokens,
+                     max(before.max_len, mine.max_len)};
+        if (lane == 0) {
+            st_state(me, pack_lo(kPrefix, incl), kPrefix | incl.tokens);
+            sm.base_count = before.count;
+            sm.base_tokens = before.tokens;
+            if (tile == 0) p.cu_seqlens[0] = 0;
+            if (tile == p.num_tiles - 1) {
+                *p.n_survivors = (int32_t)incl.count;
+                *p.total_tokens = (int64_t)incl.tokens;
+                *p.max_seqlen = incl.max_len;
+            }
+        }
+    }
+    __syncthreads();
+
+    // Four items at a time so that their (independent) warp scans overlap.
+    const u64 base_c = sm.base_count, base_t = sm.base_tokens;
+    constexpr int U = 4;
+    for (int k0 = 0; k0 < items; k0 += U) {
+        int v[U];
+        unsigned ballot[U];
+        uint32_t x[U];
+        uint32_t mx = 0;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            v[u] = (k0 + u < items) ? sm.len[(k0 + u) * kThreads + tid] : -1;
+            ballot[u] = __ballot_sync(0xffffffffu, v[u] >= 0);
+            x[u] = v[u] >= 0 ? (uint32_t)v[u] : 0u;
+            mx = max(mx, x[u]);
+        }
+        const bool small = __reduce_max_sync(0xffffffffu, mx) < (1u << 26);  // 32 lanes cannot overflow
+        u64 incl[U];
+        if (small) {
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const uint32_t y = __shfl_up_sync(0xffffffffu, x[u], o);
+                    if (lane >= o) x[u] += y;
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) incl[u] = x[u];
+        } else {
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                u64 z = x[u];
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const u64 y = __shfl_up_sync(0xffffffffu, z, o);
+                    if (lane >= o) z += y;
+                }
+                incl[u] = z;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (v[u] >= 0) {
+                const int k = k0 + u;
+                const unsigned rank = __popc(ballot[u] & ((1u << lane) - 1u));
+                const u64 r = base_c + sm.part_count[k * kWarps + warp] + rank;
+                p.survivor_idx[r] = (int32_t)(q0 + (int64_t)k * kThreads + tid);
+                p.cu_seqlens[r + 1] = (int64_t)(base_t + sm.part_tokens[k * kWarps + warp] + incl[u]);
+            }
+        }
+    }
+}
 
 template <int E_T, int CONF, bool DO_GATE, bool DO_COMPACT, int MAXI, int BATCH>
 __global__ void __launch_bounds__(kThreads, kBlocksPerSM) gate_compact_kernel(const GateArgs p) {
@@ -382,112 +530,7 @@ __global__ void __launch_bounds__(kThreads, kBlocksPerSM) gate_compact_kernel(co
         }
     }
 
-    if constexpr (DO_COMPACT) {
-        // ---- G4-G5: stable compaction and cu_seqlens -------------------------------------------
-        // Scan order inside the tile is (item, thread): exactly ascending question index.
-        my_max = __reduce_max_sync(0xffffffffu, my_max);
-        if (lane == 0) sm.warp_max[warp] = my_max;
-        __syncthreads();
-
-        if (warp == 0) {
-            // exclusive scan of the items * kWarps (<= 128) partials, 4 consecutive per lane
-            constexpr int PER = (MAXI * kWarps + 31) / 32;
-            const int n_part = items * kWarps;
-            unsigned int c[PER];
-            u64 t[PER];
-            unsigned int csum = 0;
-            u64 tsum = 0;
-#pragma unroll
-            for (int j = 0; j < PER; ++j) {
-                const int e = lane * PER + j;
-                c[j] = e < n_part ? sm.part_count[e] : 0u;
-                t[j] = e < n_part ? sm.part_tokens[e] : 0ull;
-                csum += c[j];
-                tsum += t[j];
-            }
-            unsigned int ci = csum;
-            u64 ti = tsum;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const unsigned int cc = __shfl_up_sync(0xffffffffu, ci, o);
-                const u64 tt = __shfl_up_sync(0xffffffffu, ti, o);
-                if (lane >= o) {
-                    ci += cc;
-                    ti += tt;
-                }
-            }
-            unsigned int cx = ci - csum;
-            u64 tx = ti - tsum;
-#pragma unroll
-            for (int j = 0; j < PER; ++j) {
-                const int e = lane * PER + j;
-                if (e < n_part) {
-                    sm.part_count[e] = cx;
-                    sm.part_tokens[e] = tx;
-                }
-                cx += c[j];
-                tx += t[j];
-            }
-            Partial mine;
-            mine.count = __shfl_sync(0xffffffffu, ci, 31);
-            mine.tokens = __shfl_sync(0xffffffffu, ti, 31);
-            mine.max_len = __reduce_max_sync(0xffffffffu, lane < kWarps ? sm.warp_max[lane] : 0);
-
-            TileState* me = p.tiles + tile;
-            Partial before{0, 0, 0};
-            if (tile != 0) {
-                if (lane == 0) st_state(me, pack_lo(kAggregate, mine), kAggregate | mine.tokens);
-                before = look_back(p.tiles, (int)tile, lane);
-            }
-            Partial incl{before.count + mine.count, before.tokens + mine.tokens,
-                         max(before.max_len, mine.max_len)};
-            if (lane == 0) {
-                st_state(me, pack_lo(kPrefix, incl), kPrefix | incl.tokens);
-                sm.base_count = before.count;
-                sm.base_tokens = before.tokens;
-                if (tile == 0) p.cu_seqlens[0] = 0;
-                if (tile == p.num_tiles - 1) {
-                    *p.n_survivors = (int32_t)incl.count;
-                    *p.total_tokens = (int64_t)incl.tokens;
-                    *p.max_seqlen = incl.max_len;
-                }
-            }
-        }
-        __syncthreads();
-
-        const u64 base_c = sm.base_count, base_t = sm.base_tokens;
-        for (int k = 0; k < items; ++k) {
-            const int v = sm.len[k * kThreads + tid];
-            const bool s = v >= 0;
-            const unsigned ballot = __ballot_sync(0xffffffffu, s);
-            if (ballot == 0) continue;
-            const unsigned rank = __popc(ballot & ((1u << lane) - 1u));
-            u64 incl;
-            const uint32_t vv = s ? (uint32_t)v : 0u;
-            if (__reduce_max_sync(0xffffffffu, vv) < (1u << 26)) {  // 32 lanes cannot overflow
-                uint32_t x = vv;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
-                    if (lane >= o) x += y;
-                }
-                incl = x;
-            } else {
-                u64 x = vv;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const u64 y = __shfl_up_sync(0xffffffffu, x, o);
-                    if (lane >= o) x += y;
-                }
-                incl = x;
-            }
-            if (s) {
-                const u64 r = base_c + sm.part_count[k * kWarps + warp] + rank;
-                p.survivor_idx[r] = (int32_t)(q0 + (int64_t)k * kThreads + tid);
-                p.cu_seqlens[r + 1] = (int64_t)(base_t + sm.part_tokens[k * kWarps + warp] + incl);
-            }
-        }
-    }
+    if constexpr (DO_COMPACT) compact_tile<MAXI>(p, sm, tile, q0, items, my_max);
 }
 
 // Questions per thread: as many as needed for the grid to be one co-resident wave
@@ -659,3 +702,5 @@ extern "C" mosaic_status_t mosaic_gate_compact(
                ? dispatch_gate<MOSAIC_CONF_WEIGHTED, true>(a, workspace_bytes, workspace, s)
                : dispatch_gate<MOSAIC_CONF_VOTE, true>(a, workspace_bytes, workspace, s);
 }
+
+
