@@ -53,6 +53,27 @@ def gate_bytes_per_query(E, weighted, survive_frac):
     return 4 * E * (2 if weighted else 1) + 4 + (4 + 4 + 1) + survive_frac * (4 + 8)
 
 
+def whole_job(secs: float, units: float, world: int, device="cpu"):
+    """Whole-job aggregate over the ranks: (max over ranks of the timed seconds, sum over ranks of
+    the units processed).  Weak scaling, no data-path collective: every rank works on its own
+    batch, these two reductions are the only communication.  Works on any backend (gloo on CPU in
+    tests/test_multi_rank.py, nccl in the bench)."""
+    if world <= 1:
+        return float(secs), float(units)
+    import torch
+    import torch.distributed as dist
+    mx = torch.tensor([secs], dtype=torch.float64, device=device)
+    sm = torch.tensor([units], dtype=torch.float64, device=device)
+    dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+    dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+    return float(mx[0]), float(sm[0])
+
+
+def rank_seed(rank: int) -> int:
+    """Seed of the batch rank `rank` generates for itself (weak scaling: one batch per rank)."""
+    return int(rank)
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -245,7 +266,7 @@ def run_product(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     pk, pk_src = peaks()
     cfg = wl.C2
-    seed = rank  # weak scaling: every rank gates and attends its own batch, no collective
+    seed = rank_seed(rank)  # weak scaling: every rank gates and attends its own batch, no collective
     gi = wl.gate_inputs(cfg, seed)
     a = torch.from_numpy(gi.answers).cuda()
     cl = torch.from_numpy(gi.ctx_len).cuda()
@@ -295,14 +316,7 @@ def run_product(args):
     clocks = sampler.stop() if sampler else None
     secs = t0.elapsed_time(t1) * 1e-3
     attn_ms = float(np.mean([e0.elapsed_time(e1) for e0, e1 in ev_attn]))
-    tot = torch.tensor([secs, flops * args.steps], dtype=torch.float64, device="cuda")
-    if world > 1:
-        mx = tot.clone()
-        dist.all_reduce(mx, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-        secs_max, flops_all = float(mx[0]), float(tot[1])
-    else:
-        secs_max, flops_all = secs, float(tot[1])
+    secs_max, flops_all = whole_job(secs, flops * args.steps, world, "cuda")
     value = flops_all / secs_max / 1e12
 
     # ---- end to end through the host-buffer call (pinned host memory, copies timed) ----------
@@ -330,9 +344,8 @@ def run_product(args):
     barrier()
     e2e_secs = max(e0.elapsed_time(e1) * 1e-3, 0.0)
     e2e_wall = time.perf_counter() - w0
-    tt = torch.tensor([e2e_secs], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    e2e_max, _ = whole_job(e2e_secs, 0.0, world, "cuda")
+    tt = [e2e_max]
     e2e_value = flops_all / args.steps * e2e_steps / float(tt[0]) / 1e12
     h2d = gi.answers.nbytes + gi.ctx_len.nbytes + (qh.numel() + kh.numel() + vh.numel()) * 2
     d2h = (16 + cfg.Q * 9 + S * 4 + (S + 1) * 8 + T * cfg.Hq * cfg.D * 2 + T * cfg.Hq * 4)
