@@ -84,7 +84,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                       "--format=csv,noheader,nounits", "-lms", "20"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -241,12 +241,16 @@ def bench_gate_c5(torch, mosaic, wl, pk, steps, warmup):
     ms = np.array([e0.elapsed_time(e1) for e0, e1 in evs]) / nsets
     t = float(np.mean(ms)) * 1e-3
     gbs = bytes_per_call / t / 1e9
+    traffic = None
+    tj = ROOT / "profiles" / "traffic.json"
+    if tj.exists():
+        traffic = json.loads(tj.read_text()).get("gate_compact_dram_bytes_per_launch")
     return {"workload": "C5-large-sweep gate+compaction: Q=2^20, E=8, weighted conf, p=0.6, tau=0.75",
             "call": "mosaic_gate_compact (memset + 1 kernel), CUDA-graph replay of 4 calls", "mqueries_per_s": cfg.Q / t / 1e6,
             "us_per_call": t * 1e6, "us_best": float(ms.min()) * 1e3, "survivors": S,
             "l2": "cold: 4 buffer sets (~93 MB each) used round-robin",
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                         "frac": gbs / pk["hbm_gbs"], "traffic": None,
+                         "frac": gbs / pk["hbm_gbs"], "traffic": traffic,
                          "algorithmic_bytes": bytes_per_call}}
 
 
