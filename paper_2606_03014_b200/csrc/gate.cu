@@ -237,6 +237,8 @@ struct GateArgs {
     int32_t* max_seqlen;
     ScanHeader* header;
     TileState* tiles;
+    int tile_stride;  // tile t lives at tiles[t * tile_stride]: one state per 128-byte line when the
+                      // workspace allows, so the look-back loads of ~300 tiles spread over the L2 slices
     unsigned int num_tiles;
     int items;  // questions per thread in this launch
 };
@@ -246,7 +248,7 @@ struct GateArgs {
 // including its first inclusive prefix; lanes before the first lane that met a prefix count in
 // full, that lane counts its partial sum, later lanes do not count.  With the grid a single wave
 // of <= 296 tiles this is one round of loads.  Whole warp calls; result in every lane.
-__device__ __forceinline__ Partial look_back(const TileState* tiles, int tile, int lane) {
+__device__ __forceinline__ Partial look_back(const TileState* tiles, int stride, int tile, int lane) {
     constexpr int W = 8;
     Partial acc{0, 0, 0};
     bool done = false;
@@ -265,7 +267,7 @@ __device__ __forceinline__ Partial look_back(const TileState* tiles, int tile, i
             for (int j = 0; j < W; ++j) {
                 const int idx = base - (lane * W + j);
                 const bool ready = (lo[j] >> 62) != 0 && (lo[j] >> 62) == (hi[j] >> 62);
-                if (!ready) ld_state(tiles + idx, lo[j], hi[j]);
+                if (!ready) ld_state(tiles + (size_t)idx * stride, lo[j], hi[j]);
             }
             pending = false;
 #pragma unroll
@@ -372,11 +374,11 @@ __device__ __forceinline__ void compact_tile(const GateArgs& p, GateSmem<MAXI>& 
         mine.tokens = __shfl_sync(0xffffffffu, ti, 31);
         mine.max_len = __reduce_max_sync(0xffffffffu, lane < kWarps ? sm.warp_max[lane] : 0);
 
-        TileState* me = p.tiles + tile;
+        TileState* me = p.tiles + (size_t)tile * p.tile_stride;
         Partial before{0, 0, 0};
         if (tile != 0) {
             if (lane == 0) st_state(me, pack_lo(kAggregate, mine), kAggregate | mine.tokens);
-            before = look_back(p.tiles, (int)tile, lane);
+            before = look_back(p.tiles, p.tile_stride, (int)tile, lane);
         }
         Partial incl{before.count + mine.count, before.tokens + mine.tokens,
                      max(before.max_len, mine.max_len)};
@@ -550,7 +552,11 @@ mosaic_status_t launch(GateArgs& a, size_t ws_bytes, void* workspace, cudaStream
     const unsigned int tiles = (unsigned int)((a.Q + tile - 1) / tile);
     a.num_tiles = tiles;
     if constexpr (DO_COMPACT) {
-        const size_t need = sizeof(ScanHeader) + (size_t)tiles * sizeof(TileState);
+        int stride = 8;  // 128-byte lines if the workspace holds them, else denser
+        while (stride > 1 && sizeof(ScanHeader) + (size_t)tiles * stride * sizeof(TileState) > ws_bytes)
+            stride >>= 1;
+        a.tile_stride = stride;
+        const size_t need = sizeof(ScanHeader) + (size_t)tiles * stride * sizeof(TileState);
         if (ws_bytes < need) return MOSAIC_ERR_WORKSPACE_TOO_SMALL;
         a.header = static_cast<ScanHeader*>(workspace);
         a.tiles = reinterpret_cast<TileState*>(static_cast<char*>(workspace) + sizeof(ScanHeader));
