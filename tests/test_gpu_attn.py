@@ -120,6 +120,21 @@ def _config_batch(cfg, seed):
     return oc["cu_seqlens"][:n + 1]
 
 
+@pytest.mark.parametrize("seed", [1, 2])
+def test_c2_other_seeds_sampled_rows(seed):
+    """The bench config on the paper's other two seeds: sampled rows against the oracle."""
+    cfg = wl.C2
+    gi = wl.gate_inputs(cfg, seed)
+    oc = oracle.compact(oracle.gate(gi.answers, gi.tau)["bypass"], gi.ctx_len)
+    cu = oc["cu_seqlens"]
+    q, k, v = wl.qkv(cfg, seed, int(cu[-1]), device="cuda")
+    scale = wl.softmax_scale(cfg)
+    o, lse = P.run_attn(q, k, v, cu, scale)
+    rs, rh, rp = wl.sample_rows(cu, cfg.Hq, cfg.Hkv, seed, cfg.config_id, n_random=512)
+    eo, el = P.check_attn_rows(o, lse, q, k, v, cu, rs, rh, rp, scale)
+    assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
+
+
 @pytest.mark.parametrize("cid,n_random", [(2, 1024), (3, 512), (4, 1024), (5, 256)])
 def test_configs_sampled_rows_and_structured(cid, n_random):
     """BASELINE configs[1..4] at full size, in the launch configuration bench.py times: sampled
