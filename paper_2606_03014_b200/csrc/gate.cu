@@ -67,6 +67,18 @@ __device__ __forceinline__ void st_state(TileState* s, u64 lo, u64 hi) {
     asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(s), "l"(lo), "l"(hi) : "memory");
 }
 
+// Programmatic dependent launch: the kernel that zeroes the scan workspace is launched just before
+// this one and the two overlap; every thread that touches the workspace first waits here for the
+// zeroing grid to have completed (and its writes to be visible).
+__device__ __forceinline__ void wait_for_workspace() {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
+__global__ void __launch_bounds__(256) zero_workspace_kernel(uint4* p, size_t n16) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n16) p[i] = make_uint4(0u, 0u, 0u, 0u);
+}
+
 // Row loads.  Rows start 16-byte aligned when E % 4 == 0 (32-byte when E % 8 == 0) because the
 // base pointer is; 32-byte rows use one 256-bit load, streamed past L1.
 template <int E_T, int EM, typename T>
@@ -237,6 +249,7 @@ struct GateArgs {
     int32_t* max_seqlen;
     ScanHeader* header;
     TileState* tiles;
+    int use_ticket;   // tiles numbered by an atomic ticket (grids of more than one wave), else by blockIdx
     int tile_stride;  // tile t lives at tiles[t * tile_stride]: one state per 128-byte line when the
                       // workspace allows, so the look-back loads of ~300 tiles spread over the L2 slices
     unsigned int num_tiles;
@@ -374,6 +387,7 @@ __device__ __forceinline__ void compact_tile(const GateArgs& p, GateSmem<MAXI>& 
         mine.tokens = __shfl_sync(0xffffffffu, ti, 31);
         mine.max_len = __reduce_max_sync(0xffffffffu, lane < kWarps ? sm.warp_max[lane] : 0);
 
+        wait_for_workspace();  // (returns at once when the zeroing grid is already complete)
         TileState* me = p.tiles + (size_t)tile * p.tile_stride;
         Partial before{0, 0, 0};
         if (tile != 0) {
@@ -460,7 +474,14 @@ __global__ void __launch_bounds__(kThreads, kBlocksPerSM) gate_compact_kernel(co
 
     unsigned int tile = blockIdx.x;
     if constexpr (DO_COMPACT) {
-        if (tid == 0) sm.tile = atomicAdd(&p.header->ticket, 1u);
+        if (tid == 0) {
+            if (p.use_ticket) {
+                wait_for_workspace();
+                sm.tile = atomicAdd(&p.header->ticket, 1u);
+            } else {
+                sm.tile = blockIdx.x;
+            }
+        }
         __syncthreads();
         tile = sm.tile;
     }
@@ -560,7 +581,30 @@ mosaic_status_t launch(GateArgs& a, size_t ws_bytes, void* workspace, cudaStream
         if (ws_bytes < need) return MOSAIC_ERR_WORKSPACE_TOO_SMALL;
         a.header = static_cast<ScanHeader*>(workspace);
         a.tiles = reinterpret_cast<TileState*>(static_cast<char*>(workspace) + sizeof(ScanHeader));
-        MOSAIC_CUDA_TRY(cudaMemsetAsync(workspace, 0, need, stream));
+        // One co-resident wave: tile = blockIdx (blocks are dispatched in index order, so a tile
+        // only ever waits for tiles that are already running) and the workspace is first touched
+        // after the streaming phase, which therefore overlaps its zeroing.  Larger grids take a
+        // ticket at block start instead, and wait for the zeroing there.
+        a.use_ticket = tiles > (unsigned)(num_sms() * kBlocksPerSM) ? 1 : 0;
+        const size_t n16 = (need + 15) / 16;
+        zero_workspace_kernel<<<(unsigned)((n16 + 255) / 256), 256, 0, stream>>>(
+            static_cast<uint4*>(workspace), n16);
+        count_launch();
+        MOSAIC_CUDA_TRY(cudaGetLastError());
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(tiles);
+        cfg.blockDim = dim3(kThreads);
+        cfg.dynamicSmemBytes = 0;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        MOSAIC_CUDA_TRY(cudaLaunchKernelEx(
+            &cfg, gate_compact_kernel<E_T, CONF, DO_GATE, DO_COMPACT, MAXI, BATCH>, a));
+        count_launch();
+        return MOSAIC_OK;
     }
     gate_compact_kernel<E_T, CONF, DO_GATE, DO_COMPACT, MAXI, BATCH>
         <<<tiles, kThreads, 0, stream>>>(a);
