@@ -12,10 +12,12 @@
 //   independent streams that share only the K/V ring: each has its own MMA-issuing thread and
 //   its own softmax group, so one tile's MMAs fill the tensor pipe while the other is in
 //   softmax, and a tile that finishes its item first starts the next item without waiting.
-//     warps 0-3   : softmax + epilogue of tile 0        warps 4-7 : ... of tile 1
-//     warp 8      : TMA producer (Q tiles, K/V ring of kSlots 128-key tiles, 128-byte swizzle)
-//     warp 9, 10  : tcgen05.mma issuer of tile 0 / tile 1 (one elected thread each);
-//                   warp 10 also allocates / releases tensor memory
+//     warps 0-3   : softmax of tile 0                   warps 4-7 : ... of tile 1
+//     warps 8-11  : epilogue of both tiles (O_t / l -> bf16 -> global, logsumexp), so that the
+//                   softmax groups go straight on to the next item
+//     warp 12     : TMA producer (Q tiles, K/V ring of kSlots 128-key tiles, 128-byte swizzle)
+//     warp 13, 14 : tcgen05.mma issuer of tile 0 / tile 1 (one elected thread each);
+//                   warp 14 also allocates / releases tensor memory
 //   The two issuers take a lock around each group of MMAs so the groups alternate in the tensor
 //   pipe; a quarter of the exponentials is evaluated on the FMA pipe (exp2_poly2), the rest on MUFU.
 //   (MOSAIC_P_HALVES=1 hands P_t to the tensor core in two halves of 64 keys; off by default.)
@@ -42,11 +44,12 @@ constexpr int BQ = 2 * BM;    // query rows per work item (two tiles)
 #define MOSAIC_KV_SLOTS 5
 #endif
 constexpr int kSlots = MOSAIC_KV_SLOTS;  // K/V ring depth (tiles)
-constexpr int kThreadsAttn = 384;
+constexpr int kThreadsAttn = 512;
 // Warp roles.  The softmax groups take the LOW warp ids (TMEM lane quarter = warp % 4) and the
 // single-thread roles the HIGH ones: the warp schedulers favour the highest warp id among the
 // eligible warps, and the MMA issuers are the threads everything else waits for.
-constexpr int kWarpProducer = 8, kWarpMma0 = 9, kWarpMma1 = 10;  // warp 11: idle
+constexpr int kWarpEpilogue = 8;  // warps 8-11: O_t / l -> global, for both tiles
+constexpr int kWarpProducer = 12, kWarpMma0 = 13, kWarpMma1 = 14;  // warp 15: idle
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units
@@ -185,8 +188,9 @@ struct SmemLayout {
     static constexpr int kQ = 0;                    // Q_0, Q_1
     static constexpr int kKV = 2 * kTileBytes;      // ring of kSlots tiles
     static constexpr int kBars = kKV + kSlots * kTileBytes;
-    static constexpr int kTotal = kBars + 512;
-    static constexpr int kDynamic = kTotal + 1024;  // slack for the 1024-byte alignment
+    static constexpr int kStat = kBars + 512;       // (m, l) of every row of both tiles, for the epilogue
+    static constexpr int kTotal = kStat + 2 * BM * 8;
+    static constexpr int kDynamic = kTotal;         // the base is 1024-byte aligned (checked)
     static_assert(kDynamic <= 227 * 1024, "shared memory of one CTA");
 };
 
@@ -200,7 +204,9 @@ enum Bar : uint32_t {
     kBarPHalf = kBarSFull + 2,              // [2]  keys 0-63 of P_t written         (4 warps)
     kBarPFull = kBarSFull + 4,              // [2]  keys 64-127 of P_t written       (4 warps)
     kBarODone = kBarSFull + 6,              // [2]  last PV_t of the item complete   (commit)
-    kNumBars = kBarSFull + 8
+    kBarStat = kBarSFull + 8,               // [2]  (m, l) of the tile's rows are in shared memory (4 warps)
+    kBarOFree = kBarSFull + 10,             // [2]  the epilogue has read O_t        (4 warps)
+    kNumBars = kBarSFull + 12
 };
 static_assert(kNumBars * 8 + 8 <= 512, "barrier region");
 
@@ -267,9 +273,9 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
     using SL = SmemLayout<D>;
     constexpr int kTmemCols = 512;  // S_0/P_0: [0,128)  S_1/P_1: [128,256)  O_0: [256,..)  O_1: [384,..)
 
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-    uint8_t* smem = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
+    extern __shared__ __align__(1024) uint8_t smem[];  // 128-byte swizzle wants 1024-byte alignment
+    const uint32_t smem_base = ptx::smem_u32(smem);
+    if (smem_base & 1023u) __trap();
     const uint32_t sQ = smem_base + SL::kQ, sKV = smem_base + SL::kKV;
     const uint32_t bars = smem_base + SL::kBars;
     auto bar = [&](uint32_t which, int i = 0) { return bars + 8u * (which + (uint32_t)i); };
@@ -292,6 +298,8 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             ptx::mbar_init(bar(kBarPHalf, t), BM / 32);
             ptx::mbar_init(bar(kBarPFull, t), BM / 32);
             ptx::mbar_init(bar(kBarODone, t), 1);
+            ptx::mbar_init(bar(kBarStat, t), BM / 32);
+            ptx::mbar_init(bar(kBarOFree, t), BM / 32);
             for (int s = 0; s < kSlots; ++s) ptx::mbar_init(bar_kv_empty(t, s), 1);
         }
         for (int s = 0; s < kSlots; ++s) ptx::mbar_init(bar(kBarKvFull, s), 1);
@@ -312,9 +320,69 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
     auto slot_of = [](uint32_t q) { return q % kSlots; };
     auto phase_of = [](uint32_t q) { return (q / kSlots) & 1u; };
 
-    if (warp >= 8) {
-        setmaxnreg_dec<80>();
-        if (warp == kWarpProducer) {
+    if (warp >= kWarpEpilogue) {
+        setmaxnreg_dec<48>();
+        if (warp < kWarpProducer) {
+            // ====================== epilogue: O_t / l -> bf16 -> global; A4: logsumexp ======================
+            const int row = tid & (BM - 1);  // query row inside the tile == TMEM lane (warp % 4 quarter)
+            const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
+            const float2* stat = reinterpret_cast<const float2*>(smem + SL::kStat);
+            uint32_t ph[2] = {0, 0};
+            Work next_k{};
+            if ((int)blockIdx.x < n_work) next_k = decode_work(p, blockIdx.x);
+            for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
+                const Work k = next_k;
+                if (w + (int)gridDim.x < n_work) next_k = decode_work(p, w + gridDim.x);
+#pragma unroll 1
+                for (int t = 0; t < 2; ++t) {
+                    if (k.n[t] == 0) continue;
+                    ptx::mbar_wait(bar(kBarStat, t), ph[t]);   // the softmax group is done with the item
+                    ptx::mbar_wait(bar(kBarODone, t), ph[t]);  // ... and so is the last PV_t
+                    ph[t] ^= 1;
+                    ptx::tc_fence_after();
+                    const float2 ml = stat[t * BM + row];
+                    const uint32_t tO = tmem + 256 + t * 128 + lane_off;
+                    const int row_g = k.row0 + t * BM + row;
+                    const float inv_l = 1.f / ml.y;
+                    __nv_bfloat16* orow = p.o + ((k.t0 + row_g) * p.Hq + k.h) * (int64_t)D;
+#pragma unroll
+                    for (int c = 0; c < D / 16; ++c) {
+                        uint32_t r[16];
+                        ptx::tmem_ld16(tO + c * 16, r);
+                        ptx::tmem_wait_ld();
+                        if (row_g < k.L) {
+                            uint32_t pk[8];
+#pragma unroll
+                            for (int i = 0; i < 16; i += 2) {
+                                __nv_bfloat162 h = __floats2bfloat162_rn(
+                                    __uint_as_float(r[i]) * inv_l, __uint_as_float(r[i + 1]) * inv_l);
+                                pk[i / 2] = *reinterpret_cast<uint32_t*>(&h);
+                            }
+                            // one full 32-byte sector per store when the row is 32-byte aligned; O is
+                            // written once and never read here: do not let it displace K/V in L2
+                            if (p.o_align32) {
+                                asm volatile("st.global.L1::no_allocate.L2::evict_first.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(
+                                                 orow + c * 16),
+                                             "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]), "r"(pk[4]),
+                                             "r"(pk[5]), "r"(pk[6]), "r"(pk[7])
+                                             : "memory");
+                            } else {
+                                *reinterpret_cast<uint4*>(orow + c * 16) =
+                                    make_uint4(pk[0], pk[1], pk[2], pk[3]);
+                                *reinterpret_cast<uint4*>(orow + c * 16 + 8) =
+                                    make_uint4(pk[4], pk[5], pk[6], pk[7]);
+                            }
+                        }
+                    }
+                    // O_t and the row statistics have been read: the next item may overwrite them
+                    ptx::tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(bar(kBarOFree, t));
+                    if (row_g < k.L)
+                        p.lse[(int64_t)k.h * p.T + k.t0 + row_g] = (ml.x + log2f(ml.y)) * kLn2;
+                }
+            }
+        } else if (warp == kWarpProducer) {
             // ================================ TMA producer ================================
             uint32_t pos = 0, ph_q[2] = {0, 0};
             Work next_k{};
@@ -410,7 +478,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             };
             // The whole warp walks the work list (uniform control flow keeps the descriptors in
             // uniform registers); one elected lane issues the MMAs and their commits.
-            uint32_t pos = 0, ph_q = 0, ph_p = 0;
+            uint32_t pos = 0, ph_q = 0, ph_p = 0, ph_f = 0;
             Work next_k{};
             if ((int)blockIdx.x < n_work) next_k = decode_work(p, blockIdx.x);
             for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
@@ -447,6 +515,10 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                         __syncwarp();
 #endif
                         if (more) kv_wait(kpos);
+                        if (j == 0) {  // PV_t(0) overwrites O_t: the epilogue of the previous item is done
+                            ptx::mbar_wait(bar(kBarOFree, t), ph_f ^ 1);
+                            ph_f ^= 1;
+                        }
                         ptx::mbar_wait(bar(kBarPFull, t), ph_p);
                         ph_p ^= 1;
                         ptx::tc_fence_after();
@@ -488,7 +560,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         const uint32_t tS = tmem + t * 128 + lane_off;        // S_t, overwritten by P_t (bf16)
         const uint32_t tO = tmem + 256 + t * 128 + lane_off;  // O_t
         const float sc = p.scale_log2;
-        uint32_t ph_s = 0, ph_o = 0;
+        uint32_t ph_s = 0, ph_f = 0;
 
         Work next_k{};
             if ((int)blockIdx.x < n_work) next_k = decode_work(p, blockIdx.x);
@@ -597,46 +669,14 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                 }
                 l_run += (la.x + la.y) + (lb.x + lb.y);
             }
-            // ---- epilogue: O_t / l -> bf16 -> global; A4: logsumexp ---------------------------------
-            ptx::mbar_wait(bar(kBarODone, t), ph_o);
-            ph_o ^= 1;
-            ptx::tc_fence_after();
-            const int row_g = k.row0 + t * BM + row;
-            const float inv_l = 1.f / l_run;
-            __nv_bfloat16* orow = p.o + ((k.t0 + row_g) * p.Hq + k.h) * (int64_t)D;
-#pragma unroll
-            for (int c = 0; c < D / 32; ++c) {
-                uint32_t r[32];
-                ptx::tmem_ld32(tO + c * 32, r);
-                ptx::tmem_wait_ld();
-                if (row_g < k.L) {
-                    uint32_t pk[16];
-#pragma unroll
-                    for (int i = 0; i < 32; i += 2) {
-                        __nv_bfloat162 h = __floats2bfloat162_rn(__uint_as_float(r[i]) * inv_l,
-                                                                 __uint_as_float(r[i + 1]) * inv_l);
-                        pk[i / 2] = *reinterpret_cast<uint32_t*>(&h);
-                    }
-                    // one full 32-byte sector per store when the row is 32-byte aligned
-                    if (p.o_align32) {
-#pragma unroll
-                        for (int i = 0; i < 16; i += 8)
-                            asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(
-                                             orow + c * 32 + 2 * i),
-                                         "r"(pk[i]), "r"(pk[i + 1]), "r"(pk[i + 2]), "r"(pk[i + 3]),
-                                         "r"(pk[i + 4]), "r"(pk[i + 5]), "r"(pk[i + 6]), "r"(pk[i + 7])
-                                         : "memory");
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 16; i += 4)
-                            *reinterpret_cast<uint4*>(orow + c * 32 + 2 * i) =
-                                make_uint4(pk[i], pk[i + 1], pk[i + 2], pk[i + 3]);
-                    }
-                }
-            }
-            if (row_g < k.L)
-                p.lse[(int64_t)k.h * p.T + k.t0 + row_g] = (m_used + log2f(l_run)) * kLn2;
-            ptx::tc_fence_before();
+            // ---- hand the row's (m, l) to the epilogue warps and go on to the next item -----------
+            // (first make sure the epilogue has read the previous item's pair -- it releases O_t
+            //  after that; an item of a single KV tile gets here without PV_t(0) having waited)
+            ptx::mbar_wait(bar(kBarOFree, t), ph_f ^ 1);
+            ph_f ^= 1;
+            reinterpret_cast<float2*>(smem + SL::kStat)[t * BM + row] = make_float2(m_used, l_run);
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(bar(kBarStat, t));
         }
     }
 
