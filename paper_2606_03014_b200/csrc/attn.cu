@@ -5,22 +5,26 @@
 //
 // A5    schedule_kernel : (sequence, 256-row q block) work items, longest (most KV tiles) first.
 // A1-A4 attn_fwd        : persistent, warp-specialised tcgen05 / TMEM / TMA flash attention.
-//   One CTA per SM works through (item, q head) pairs.  A q block is two 128-row tiles; for each
-//   128-key tile j the tensor core computes S_t = Q_t K_j^T into tensor memory, a 128-thread
-//   softmax group per tile (one thread per query row) turns S_t into P_t in place (bf16, same
-//   TMEM columns), and O_t += P_t V_j accumulates in tensor memory.  The two tiles are two
+//   One CTA per SM works through (item, q head) pairs.  A q block is two 128-row tiles.  Each
+//   128-key tile j is taken in two steps of 64 keys: the tensor core computes S_t = Q_t K^T for
+//   64 keys into one of TWO 64-column score buffers of the tile in tensor memory, a 128-thread
+//   softmax group per tile (one thread per query row) turns it into P_t in place (bf16, same
+//   TMEM columns), and O_t += P_t V accumulates in tensor memory.  While the group works on one
+//   buffer the scores of the next step are already being computed into the other, so a softmax
+//   group never waits for the tensor pipe in the steady state.  The two tiles are two
 //   independent streams that share only the K/V ring: each has its own MMA-issuing thread and
-//   its own softmax group, so one tile's MMAs fill the tensor pipe while the other is in
-//   softmax, and a tile that finishes its item first starts the next item without waiting.
+//   its own softmax group, and a tile that finishes its item first starts the next item
+//   without waiting.
 //     warps 0-3   : softmax of tile 0                   warps 4-7 : ... of tile 1
 //     warps 8-11  : epilogue of both tiles (O_t / l -> bf16 -> global, logsumexp), so that the
 //                   softmax groups go straight on to the next item
 //     warp 12     : TMA producer (Q tiles, K/V ring of kSlots 128-key tiles, 128-byte swizzle)
 //     warp 13, 14 : tcgen05.mma issuer of tile 0 / tile 1 (one elected thread each);
 //                   warp 14 also allocates / releases tensor memory
-//   The two issuers take a lock around each group of MMAs so the groups alternate in the tensor
-//   pipe; a quarter of the exponentials is evaluated on the FMA pipe (exp2_poly2), the rest on MUFU.
-//   (MOSAIC_P_HALVES=1 hands P_t to the tensor core in two halves of 64 keys; off by default.)
+//   Both softmax groups are busy all the time, so the FMA / ALU issue slots are as scarce as the
+//   MUFU unit: all exponentials go to MUFU (MOSAIC_POLY_PAIRS = n evaluates n of every 4 element
+//   pairs on the FMA pipe instead, exp2_poly2; measured slower here), and the two issuers do not
+//   take turns (MOSAIC_MMA_LOCK = 1 makes them; it paid when S and P shared one buffer).
 //   The running row max is only moved (and O rescaled) when it grows by more than 2^8, so the
 //   rescale of the accumulator is rare; the final 1/l normalisation makes the result exact.
 #include <cuda.h>
@@ -38,7 +42,8 @@ namespace mosaic {
 namespace {
 
 constexpr int BM = 128;       // query rows per tile  (UMMA M)
-constexpr int BN = 128;       // key rows per tile    (UMMA N of S, UMMA K of PV)
+constexpr int BN = 128;       // key rows per K/V tile (one TMA load, one ring slot)
+constexpr int BS = 64;        // keys per step         (UMMA N of S; two steps per K/V tile)
 constexpr int BQ = 2 * BM;    // query rows per work item (two tiles)
 #ifndef MOSAIC_KV_SLOTS
 #define MOSAIC_KV_SLOTS 5
@@ -53,14 +58,11 @@ constexpr int kWarpProducer = 12, kWarpMma0 = 13, kWarpMma1 = 14;  // warp 15: i
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units
-#ifndef MOSAIC_P_HALVES
-#define MOSAIC_P_HALVES 0
-#endif
 #ifndef MOSAIC_POLY_PAIRS
-#define MOSAIC_POLY_PAIRS 1
+#define MOSAIC_POLY_PAIRS 0
 #endif
 #ifndef MOSAIC_MMA_LOCK
-#define MOSAIC_MMA_LOCK 1
+#define MOSAIC_MMA_LOCK 0
 #endif
 constexpr int kPolyPairs = MOSAIC_POLY_PAIRS;  // of every 4 element pairs: exp2 on the FMA pipe
 
@@ -200,13 +202,13 @@ enum Bar : uint32_t {
     kBarQEmpty = 2,                         // [2]  last S_t of the item has read Q_t (commit)
     kBarKvFull = 4,                         // [kSlots] K_j / V_j landed             (TMA tx)
     kBarKvEmpty = 4 + kSlots,               // [2][kSlots] stream t is done with the slot
-    kBarSFull = 4 + 3 * kSlots,             // [2]  S_t complete                     (commit)
-    kBarPHalf = kBarSFull + 2,              // [2]  keys 0-63 of P_t written         (4 warps)
-    kBarPFull = kBarSFull + 4,              // [2]  keys 64-127 of P_t written       (4 warps)
-    kBarODone = kBarSFull + 6,              // [2]  last PV_t of the item complete   (commit)
-    kBarStat = kBarSFull + 8,               // [2]  (m, l) of the tile's rows are in shared memory (4 warps)
-    kBarOFree = kBarSFull + 10,             // [2]  the epilogue has read O_t        (4 warps)
-    kNumBars = kBarSFull + 12
+    kBarSFull = 4 + 3 * kSlots,             // [2][2] score buffer b of tile t complete (commit)
+    kBarPFull = kBarSFull + 4,              // [2][2] P_t written over buffer b      (4 warps)
+    kBarPvDone = kBarSFull + 8,             // [2]  a PV_t step complete             (commit)
+    kBarODone = kBarSFull + 10,             // [2]  last PV_t of the item complete   (commit)
+    kBarStat = kBarSFull + 12,              // [2]  (m, l) of the tile's rows are in shared memory (4 warps)
+    kBarOFree = kBarSFull + 14,             // [2]  the epilogue has read O_t        (4 warps)
+    kNumBars = kBarSFull + 16
 };
 static_assert(kNumBars * 8 + 8 <= 512, "barrier region");
 
@@ -220,12 +222,16 @@ struct Work {
     int n_kv;        // max of the two
 };
 
-__device__ __forceinline__ Work decode_work(const AttnParams& p, int w) {
+// The descriptor of work unit w is loaded one unit ahead and decoded only when the unit starts:
+// the load (an L2 round trip) is then hidden behind the unit before it.
+__device__ __forceinline__ int4 load_item(const AttnParams& p, int w) {
+    return __ldg(p.items + w / p.Hq);
+}
+__device__ __forceinline__ Work decode_work(const AttnParams& p, int w, const int4 it) {
     Work k;
     const int item = w / p.Hq;
     k.h = w - item * p.Hq;
     k.g = k.h / (p.Hq / p.Hkv);
-    const int4 it = __ldg(p.items + item);
     k.t0 = it.x;
     k.L = it.y;
     k.row0 = it.z * BQ;
@@ -271,7 +277,9 @@ __global__ void __launch_bounds__(kThreadsAttn, 1)
 attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
          const __grid_constant__ CUtensorMap tm_v, const AttnParams p, const int negate_q) {
     using SL = SmemLayout<D>;
-    constexpr int kTmemCols = 512;  // S_0/P_0: [0,128)  S_1/P_1: [128,256)  O_0: [256,..)  O_1: [384,..)
+    // tile t: score buffers [128 t, 128 t + 64) and [128 t + 64, 128 t + 128), each overwritten by
+    // its P (bf16, 32 columns); O_t: [256 + 128 t, ..)
+    constexpr int kTmemCols = 512;
 
     extern __shared__ __align__(1024) uint8_t smem[];  // 128-byte swizzle wants 1024-byte alignment
     const uint32_t smem_base = ptx::smem_u32(smem);
@@ -294,9 +302,11 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         for (int t = 0; t < 2; ++t) {
             ptx::mbar_init(bar(kBarQFull, t), 1);
             ptx::mbar_init(bar(kBarQEmpty, t), 1);
-            ptx::mbar_init(bar(kBarSFull, t), 1);
-            ptx::mbar_init(bar(kBarPHalf, t), BM / 32);
-            ptx::mbar_init(bar(kBarPFull, t), BM / 32);
+            for (int b = 0; b < 2; ++b) {
+                ptx::mbar_init(bar(kBarSFull, 2 * t + b), 1);
+                ptx::mbar_init(bar(kBarPFull, 2 * t + b), BM / 32);
+            }
+            ptx::mbar_init(bar(kBarPvDone, t), 1);
             ptx::mbar_init(bar(kBarODone, t), 1);
             ptx::mbar_init(bar(kBarStat, t), BM / 32);
             ptx::mbar_init(bar(kBarOFree, t), BM / 32);
@@ -328,11 +338,11 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
             const float2* stat = reinterpret_cast<const float2*>(smem + SL::kStat);
             uint32_t ph[2] = {0, 0};
-            Work next_k{};
-            if ((int)blockIdx.x < n_work) next_k = decode_work(p, blockIdx.x);
+            int4 next_it = make_int4(0, 0, 0, 0);
+            if ((int)blockIdx.x < n_work) next_it = load_item(p, blockIdx.x);
             for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-                const Work k = next_k;
-                if (w + (int)gridDim.x < n_work) next_k = decode_work(p, w + gridDim.x);
+                const Work k = decode_work(p, w, next_it);
+                if (w + (int)gridDim.x < n_work) next_it = load_item(p, w + gridDim.x);
 #pragma unroll 1
                 for (int t = 0; t < 2; ++t) {
                     if (k.n[t] == 0) continue;
@@ -385,11 +395,11 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         } else if (warp == kWarpProducer) {
             // ================================ TMA producer ================================
             uint32_t pos = 0, ph_q[2] = {0, 0};
-            Work next_k{};
-            if ((int)blockIdx.x < n_work) next_k = decode_work(p, blockIdx.x);
+            int4 next_it = make_int4(0, 0, 0, 0);
+            if ((int)blockIdx.x < n_work) next_it = load_item(p, blockIdx.x);
             for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-                const Work k = next_k;  // the next item is decoded one item ahead (L2 latency)
-                if (w + (int)gridDim.x < n_work) next_k = decode_work(p, w + gridDim.x);
+                const Work k = decode_work(p, w, next_it);
+                if (w + (int)gridDim.x < n_work) next_it = load_item(p, w + gridDim.x);
                 auto load_q = [&](int t) {
                     ptx::mbar_wait(bar(kBarQEmpty, t), ph_q[t] ^ 1);
                     ph_q[t] ^= 1;
@@ -431,37 +441,39 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             // ===================== MMA issuer of tile t = warp - kWarpMma0 =====================
             const int t = warp - kWarpMma0;
             const uint32_t idesc_s =
-                ptx::umma_idesc_bf16(BM, BN, false, false) | (negate_q ? (1u << 13) : 0u);
+                ptx::umma_idesc_bf16(BM, BS, false, false) | (negate_q ? (1u << 13) : 0u);
             constexpr uint32_t idesc_pv = ptx::umma_idesc_bf16(BM, D, false, true);
             const uint32_t tS = tmem + t * 128, tO = tmem + 256 + t * 128;
             const uint32_t q_smem = sQ + t * SL::kTileBytes;
             auto kv_wait = [&](uint32_t q) { ptx::mbar_wait(bar(kBarKvFull, slot_of(q)), phase_of(q)); };
-            // S_t = Q_t K^T : both operands K-major (D contiguous), 128-byte swizzle
+            // S_t[b] = Q_t K[64 b, 64 b + 64)^T : both operands K-major (D contiguous), 128-byte swizzle
             // (descriptors of the k-th 16-wide slice = descriptor of the tile + a constant in the
-            //  14-bit start-address field; tiles are 1024-byte aligned and < 256 KB, so no carry)
+            //  14-bit start-address field; tiles are 1024-byte aligned and < 256 KB, so no carry;
+            //  64 key rows are 8 swizzle atoms = 8192 bytes further on)
             const uint64_t q_desc = ptx::umma_smem_desc_sw128(q_smem, 16, 1024);
-            auto issue_qk = [&](uint32_t kslot) {
-                const uint64_t k_desc = ptx::umma_smem_desc_sw128(sKV + kslot * SL::kTileBytes, 16, 1024);
+            auto issue_qk = [&](uint32_t kslot, int b) {
+                const uint64_t k_desc = ptx::umma_smem_desc_sw128(
+                    sKV + kslot * SL::kTileBytes + b * (BS * 128), 16, 1024);
 #pragma unroll
                 for (int kk = 0; kk < D / 16; ++kk) {
                     constexpr int kBlk = SL::kBlockBytes;
                     const uint64_t off = (uint64_t)(((kk / 4) * kBlk + (kk % 4) * 32) >> 4);
-                    ptx::umma_ss(tS, q_desc + off, k_desc + off, idesc_s, kk > 0);
+                    ptx::umma_ss(tS + b * BS, q_desc + off, k_desc + off, idesc_s, kk > 0);
                 }
             };
-            // O_t (+)= P_t[:, 16 kk0 .. 16 kk1) V : A = P_t from tensor memory, B = V (MN-major)
-            auto issue_pv = [&](uint32_t vslot, int kk0, int kk1, bool accumulate) {
+            // O_t (+)= P_t[b] V[64 b, 64 b + 64) : A = P_t[b] from tensor memory, B = V (MN-major)
+            auto issue_pv = [&](uint32_t vslot, int b, bool accumulate) {
                 const uint64_t v_desc =
                     ptx::umma_smem_desc_sw128(sKV + vslot * SL::kTileBytes, SL::kBlockBytes, 1024);
 #pragma unroll
-                for (int kk = kk0; kk < kk1; ++kk)
-                    ptx::umma_ts(tO, tS + kk * 8, v_desc + (uint64_t)((kk * 2048) >> 4), idesc_pv,
-                                 (accumulate || kk > kk0) ? 1u : 0u);
+                for (int kk = 0; kk < BS / 16; ++kk)
+                    ptx::umma_ts(tO, tS + b * BS + kk * 8,
+                                 v_desc + (uint64_t)(((b * (BS / 16) + kk) * 2048) >> 4), idesc_pv,
+                                 (accumulate || kk > 0) ? 1u : 0u);
             };
-            // The tensor pipe runs MMAs in issue order.  Each issuer holds this lock while it
-            // issues one group of MMAs, so the groups of the two tiles alternate instead of
-            // interleaving instruction by instruction: their S tiles then complete half a step
-            // apart and the two softmax groups stay out of phase.
+            // The tensor pipe runs MMAs in issue order.  With MOSAIC_MMA_LOCK an issuer holds this
+            // lock while it issues one group of MMAs, so that the groups of the two tiles alternate
+            // instead of interleaving instruction by instruction (off: see the file header).
             auto lock = [&]() {
 #if MOSAIC_MMA_LOCK
                 uint32_t old;
@@ -478,12 +490,17 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             };
             // The whole warp walks the work list (uniform control flow keeps the descriptors in
             // uniform registers); one elected lane issues the MMAs and their commits.
+            // Steps u = 2 j + b (KV tile j, half b) of an item use score buffer b.  The scores run
+            // two steps ahead of the PVs:
+            //   S(0) S(1) | PV(0) S(2) | PV(1) S(3) | ... | PV(U-2) | PV(U-1)
+            // so S(u+2) overwrites P(u) right behind PV(u) in the (in-order) tensor pipe and is
+            // ready, as a rule, before the softmax group has finished step u + 1.
             uint32_t pos = 0, ph_q = 0, ph_p = 0, ph_f = 0;
-            Work next_k{};
-            if ((int)blockIdx.x < n_work) next_k = decode_work(p, blockIdx.x);
+            int4 next_it = make_int4(0, 0, 0, 0);
+            if ((int)blockIdx.x < n_work) next_it = load_item(p, blockIdx.x);
             for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-                const Work k = next_k;  // the next item is decoded one item ahead (L2 latency)
-                if (w + (int)gridDim.x < n_work) next_k = decode_work(p, w + gridDim.x);
+                const Work k = decode_work(p, w, next_it);
+                if (w + (int)gridDim.x < n_work) next_it = load_item(p, w + gridDim.x);
                 const int n_t = k.n[t];
                 const uint32_t base = pos;
                 if (n_t > 0) {
@@ -493,8 +510,10 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                     ptx::tc_fence_after();
                     if (ptx::elect_one()) {
                         lock();
-                        issue_qk(slot_of(base));
-                        ptx::umma_commit(bar(kBarSFull, t));
+                        issue_qk(slot_of(base), 0);
+                        ptx::umma_commit(bar(kBarSFull, 2 * t));
+                        issue_qk(slot_of(base), 1);
+                        ptx::umma_commit(bar(kBarSFull, 2 * t + 1));
                         ptx::umma_commit(bar_kv_empty(t, slot_of(base)));
                         if (n_t == 1) ptx::umma_commit(bar(kBarQEmpty, t));
                         unlock();
@@ -504,34 +523,35 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                         const uint32_t vpos = base + 2 * j + 1, kpos = vpos + 1;  // V_j, K_{j+1}
                         const bool more = j + 1 < n_t;
                         kv_wait(vpos);
-#if MOSAIC_P_HALVES
-                        ptx::mbar_wait(bar(kBarPHalf, t), ph_p);
-                        ptx::tc_fence_after();
-                        if (ptx::elect_one()) {
-                            lock();
-                            issue_pv(slot_of(vpos), 0, BN / 32, j > 0);
-                            unlock();
-                        }
-                        __syncwarp();
-#endif
                         if (more) kv_wait(kpos);
                         if (j == 0) {  // PV_t(0) overwrites O_t: the epilogue of the previous item is done
                             ptx::mbar_wait(bar(kBarOFree, t), ph_f ^ 1);
                             ph_f ^= 1;
                         }
-                        ptx::mbar_wait(bar(kBarPFull, t), ph_p);
+                        ptx::mbar_wait(bar(kBarPFull, 2 * t), ph_p);
+                        ptx::tc_fence_after();
+                        if (ptx::elect_one()) {
+                            lock();
+                            issue_pv(slot_of(vpos), 0, j > 0);
+                            ptx::umma_commit(bar(kBarPvDone, t));
+                            if (more) {
+                                issue_qk(slot_of(kpos), 0);
+                                ptx::umma_commit(bar(kBarSFull, 2 * t));
+                            }
+                            unlock();
+                        }
+                        __syncwarp();
+                        ptx::mbar_wait(bar(kBarPFull, 2 * t + 1), ph_p);
                         ph_p ^= 1;
                         ptx::tc_fence_after();
                         if (ptx::elect_one()) {
                             lock();
-                            if (MOSAIC_P_HALVES)
-                                issue_pv(slot_of(vpos), BN / 32, BN / 16, true);
-                            else
-                                issue_pv(slot_of(vpos), 0, BN / 16, j > 0);
+                            issue_pv(slot_of(vpos), 1, true);
                             ptx::umma_commit(bar_kv_empty(t, slot_of(vpos)));
+                            ptx::umma_commit(bar(kBarPvDone, t));
                             if (more) {
-                                issue_qk(slot_of(kpos));
-                                ptx::umma_commit(bar(kBarSFull, t));
+                                issue_qk(slot_of(kpos), 1);
+                                ptx::umma_commit(bar(kBarSFull, 2 * t + 1));
                                 ptx::umma_commit(bar_kv_empty(t, slot_of(kpos)));
                                 if (j + 2 == n_t) ptx::umma_commit(bar(kBarQEmpty, t));
                             } else {
@@ -557,50 +577,61 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         const int t = warp >> 2;                   // tile of this group (0 or 1)
         const int row = tid - t * BM;              // query row inside the tile == TMEM lane
         const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
-        const uint32_t tS = tmem + t * 128 + lane_off;        // S_t, overwritten by P_t (bf16)
+        const uint32_t tS = tmem + t * 128 + lane_off;        // score buffers of tile t, P_t in place
         const uint32_t tO = tmem + 256 + t * 128 + lane_off;  // O_t
+        const int wq = warp & 3;                              // rows 32 wq .. 32 wq + 31 of the tile
         const float sc = p.scale_log2;
         uint32_t ph_s = 0, ph_f = 0;
+        float m_used = 0.f, l_run = 0.f;
 
-        Work next_k{};
-            if ((int)blockIdx.x < n_work) next_k = decode_work(p, blockIdx.x);
-        for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-            const Work k = next_k;  // the next item is decoded one item ahead (L2 latency)
-            if (w + (int)gridDim.x < n_work) next_k = decode_work(p, w + gridDim.x);
-            const int n_t = k.n[t];
-            if (n_t == 0) continue;  // this tile has no rows in this block
-            float m_used = 0.f, l_run = 0.f;
-            for (int j = 0; j < n_t; ++j) {
-                ptx::mbar_wait(bar(kBarSFull, t), ph_s);
-                ph_s ^= 1;
-                ptx::tc_fence_after();
-                // ---- A2: scores of this row, running max -------------------------------------
-                float s[BN];
+        // One step: 64 scores of this row (buffer b) -> running max -> P (bf16, in place) -> row sum.
+        //   kMask 0: no key masked   1: keys 64 b + c > row masked   2: every key masked (warp-uniform)
+        auto step = [&](auto buf, auto mask_kind, bool first) {
+            constexpr int b = decltype(buf)::value;
+            constexpr int kMask = decltype(mask_kind)::value;
+            const uint32_t tSb = tS + b * BS;
+            ptx::mbar_wait(bar(kBarSFull, 2 * t + b), ph_s);
+            ptx::tc_fence_after();
+            if constexpr (kMask == 2) {
+                // rows 0-63 against keys 64-127 of the diagonal tile: P = 0
+                uint32_t z[16];
 #pragma unroll
-                for (int c = 0; c < BN / 32; ++c)
-                    ptx::tmem_ld32(tS + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
+                for (int i = 0; i < 16; ++i) z[i] = 0u;
+                ptx::tmem_st16(tSb, z);
+                ptx::tmem_st16(tSb + 16, z);
+            } else {
+                // ---- A2: scores of this row, running max ---------------------------------------
+                float s[BS];
+#pragma unroll
+                for (int c = 0; c < BS / 32; ++c)
+                    ptx::tmem_ld32(tSb + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
                 ptx::tmem_wait_ld();
-                const bool diag = (j == n_t - 1);  // diagonal tile: keys after the query are masked
-                if (diag) {
+                if constexpr (kMask == 1) {
 #pragma unroll
-                    for (int c = 0; c < BN; ++c)
-                        if (c > row) s[c] = -INFINITY;
+                    for (int c = 0; c < BS; ++c)
+                        if (c + b * BS > row) s[c] = -INFINITY;
                 }
                 float mx0 = s[0], mx1 = s[1], mx2 = s[2], mx3 = s[3];
 #pragma unroll
-                for (int c = 4; c < BN; c += 4) {
+                for (int c = 4; c < BS; c += 4) {
                     mx0 = fmaxf(mx0, s[c]);
                     mx1 = fmaxf(mx1, s[c + 1]);
                     mx2 = fmaxf(mx2, s[c + 2]);
                     mx3 = fmaxf(mx3, s[c + 3]);
                 }
                 const float m_new = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * sc;
-                if (j == 0) {
+                if (first) {
                     m_used = m_new;
                 } else {
                     // move the max (and rescale l, O) only when it grew by more than 2^8
                     const bool need = m_new > m_used + kRescaleThreshold;
                     if (__any_sync(0xffffffffu, need)) {
+                        // O_t must hold every PV up to the previous step (this one has not been
+                        // issued: it needs the P written below).  The barrier has completed the
+                        // phase before that one for certain (S of this step was issued behind it),
+                        // so the parity of the previous step's phase is unambiguous: it is b ^ 1.
+                        ptx::mbar_wait(bar(kBarPvDone, t), (uint32_t)(b ^ 1));
+                        ptx::tc_fence_after();
                         const float alpha = need ? ex2_approx(m_used - m_new) : 1.f;
                         if (need) m_used = m_new;
                         l_run *= alpha;
@@ -616,59 +647,76 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                         }
                     }
                 }
-                // ---- P = exp2(s * scale_log2 - m), row sum, bf16 pairs into the S columns ------
+                // ---- P = exp2(s * scale_log2 - m), row sum, bf16 pairs into the score columns ----
                 // Two elements at a time (packed fp32 FMA / ADD).  Of every four pairs, kPolyPairs
-                // are exponentiated on the FMA pipe (exp2_poly2) and the rest on the MUFU unit, whose
-                // 16 results per clock per SM would otherwise bound the whole kernel.
+                // are exponentiated on the FMA pipe (exp2_poly2) and the rest on the MUFU unit
+                // (16 results per clock per SM; DESIGN.md says why kPolyPairs is 0).
                 float2 la = make_float2(0.f, 0.f), lb = make_float2(0.f, 0.f);
                 const float2 sc2 = make_float2(sc, sc), nm2 = make_float2(-m_used, -m_used);
-                auto exp_half = [&](auto is_diag, int c0) {
-                    constexpr bool kDiag = decltype(is_diag)::value;
 #pragma unroll
-                    for (int c = c0; c < c0 + BN / 64; ++c) {
-                        uint32_t pk[16];
+                for (int c = 0; c < BS / 32; ++c) {
+                    uint32_t pk[16];
 #pragma unroll
-                        for (int i = 0; i < 32; i += 2) {
-                            const float x0 = s[c * 32 + i], x1 = s[c * 32 + i + 1];
-                            float2 e;
-                            if constexpr (kDiag) {
-                                // a masked key must give exactly 0 even when scale_log2 == 0 (-inf * 0)
-                                const float a0 = fmaf(x0, sc, -m_used), a1 = fmaf(x1, sc, -m_used);
-                                e.x = ex2_approx(x0 == -INFINITY ? -INFINITY : a0);
-                                e.y = ex2_approx(x1 == -INFINITY ? -INFINITY : a1);
-                            } else {
-                                const float2 a = __ffma2_rn(make_float2(x0, x1), sc2, nm2);
-                                if (((i >> 1) & 3) < kPolyPairs)
-                                    e = exp2_poly2(a);
-                                else
-                                    e = make_float2(ex2_approx(a.x), ex2_approx(a.y));
-                            }
-                            if ((i >> 1) & 1)
-                                lb = __fadd2_rn(lb, e);
+                    for (int i = 0; i < 32; i += 2) {
+                        const float x0 = s[c * 32 + i], x1 = s[c * 32 + i + 1];
+                        float2 e;
+                        if constexpr (kMask == 1) {
+                            // a masked key must give exactly 0 even when scale_log2 == 0 (-inf * 0)
+                            const float a0 = fmaf(x0, sc, -m_used), a1 = fmaf(x1, sc, -m_used);
+                            e.x = ex2_approx(x0 == -INFINITY ? -INFINITY : a0);
+                            e.y = ex2_approx(x1 == -INFINITY ? -INFINITY : a1);
+                        } else {
+                            const float2 a = __ffma2_rn(make_float2(x0, x1), sc2, nm2);
+                            if (((i >> 1) & 3) < kPolyPairs)
+                                e = exp2_poly2(a);
                             else
-                                la = __fadd2_rn(la, e);
-                            __nv_bfloat162 h = __floats2bfloat162_rn(e.x, e.y);
-                            pk[i / 2] = *reinterpret_cast<uint32_t*>(&h);
+                                e = make_float2(ex2_approx(a.x), ex2_approx(a.y));
                         }
-                        ptx::tmem_st16(tS + c * 16, pk);
+                        if ((i >> 1) & 1)
+                            lb = __fadd2_rn(lb, e);
+                        else
+                            la = __fadd2_rn(la, e);
+                        __nv_bfloat162 h = __floats2bfloat162_rn(e.x, e.y);
+                        pk[i / 2] = *reinterpret_cast<uint32_t*>(&h);
                     }
-                    // this half of P_t is in tensor memory: hand it to the MMA issuer
-                    if (MOSAIC_P_HALVES || c0 != 0) {
-                        ptx::tmem_wait_st();
-                        ptx::tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) ptx::mbar_arrive(bar(c0 == 0 ? kBarPHalf : kBarPFull, t));
-                    }
-                };
-                if (diag) {
-                    exp_half(std::true_type{}, 0);
-                    exp_half(std::true_type{}, BN / 64);
-                } else {
-                    exp_half(std::false_type{}, 0);
-                    exp_half(std::false_type{}, BN / 64);
+                    ptx::tmem_st16(tSb + c * 16, pk);
                 }
                 l_run += (la.x + la.y) + (lb.x + lb.y);
             }
+            // P_t[b] is in tensor memory: hand it to the MMA issuer
+            ptx::tmem_wait_st();
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(bar(kBarPFull, 2 * t + b));
+        };
+        using B0 = std::integral_constant<int, 0>;
+        using B1 = std::integral_constant<int, 1>;
+        using B2 = std::integral_constant<int, 2>;
+
+        int4 next_it = make_int4(0, 0, 0, 0);
+        if ((int)blockIdx.x < n_work) next_it = load_item(p, blockIdx.x);
+        for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
+            const Work k = decode_work(p, w, next_it);
+            if (w + (int)gridDim.x < n_work) next_it = load_item(p, w + gridDim.x);
+            const int n_t = k.n[t];
+            if (n_t == 0) continue;  // this tile has no rows in this block
+            m_used = 0.f;
+            l_run = 0.f;
+            for (int j = 0; j + 1 < n_t; ++j) {
+                step(B0{}, B0{}, j == 0);
+                step(B1{}, B0{}, false);
+                ph_s ^= 1;
+            }
+            // diagonal tile: key 64 b + c is masked for query row r when 64 b + c > r.  Per warp
+            // (32 rows) a 64-key half is either untouched, partly masked or masked altogether.
+            if (wq >= 2) {
+                step(B0{}, B0{}, n_t == 1);
+                step(B1{}, B1{}, false);
+            } else {
+                step(B0{}, B1{}, n_t == 1);
+                step(B1{}, B2{}, false);
+            }
+            ph_s ^= 1;
             // ---- hand the row's (m, l) to the epilogue warps and go on to the next item -----------
             // (first make sure the epilogue has read the previous item's pair -- it releases O_t
             //  after that; an item of a single KV tile gets here without PV_t(0) having waited)

@@ -53,6 +53,18 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
+// Non-blocking probe of the same condition.
+__device__ __forceinline__ bool mbar_test_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
 // Waits for the phase with the given parity to complete.  A wait that would never end is a bug
 // in the pipeline protocol: trap instead of hanging the GPU (MOSAIC_SPIN_LIMIT try_waits, each of
 // which already sleeps in hardware for up to ~microseconds).
@@ -89,6 +101,13 @@ __device__ __forceinline__ void tma_load_3d_hint(uint32_t smem_dst, const void* 
         ::"r"(smem_dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(bar), "r"(c0), "r"(c1), "r"(c2),
         "l"(policy)
         : "memory");
+}
+// The same box, only as far as L2 (no shared-memory destination, no barrier).
+__device__ __forceinline__ void tma_prefetch_3d(const void* tmap, int32_t c0, int32_t c1,
+                                                int32_t c2) {
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];"
+                 ::"l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
 }
 
 // 1-D bulk copy global -> shared (16-byte aligned addresses, size a multiple of 16); completes
