@@ -586,8 +586,10 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
 
         // One step: 64 scores of this row (buffer b) -> running max -> P (bf16, in place) -> row sum.
         //   kMask 0: no key masked   1: keys 64 b + c > row masked   2: every key masked (warp-uniform)
-        auto step = [&](auto buf, auto mask_kind, bool first) {
-            constexpr int b = decltype(buf)::value;
+        // (Every call site is a copy of ~500 unrolled instructions and the instruction cache is
+        //  small: the steady state gets one copy per buffer with b a constant, the two steps of
+        //  the diagonal tile share one masked copy with b a run-time value.)
+        auto step = [&](auto mask_kind, const int b, const bool first) {
             constexpr int kMask = decltype(mask_kind)::value;
             const uint32_t tSb = tS + b * BS;
             ptx::mbar_wait(bar(kBarSFull, 2 * t + b), ph_s);
@@ -609,7 +611,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                 if constexpr (kMask == 1) {
 #pragma unroll
                     for (int c = 0; c < BS; ++c)
-                        if (c + b * BS > row) s[c] = -INFINITY;
+                        if (c > row - b * BS) s[c] = -INFINITY;
                 }
                 float mx0 = s[0], mx1 = s[1], mx2 = s[2], mx3 = s[3];
 #pragma unroll
@@ -689,9 +691,9 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(bar(kBarPFull, 2 * t + b));
         };
-        using B0 = std::integral_constant<int, 0>;
-        using B1 = std::integral_constant<int, 1>;
-        using B2 = std::integral_constant<int, 2>;
+        using M0 = std::integral_constant<int, 0>;
+        using M1 = std::integral_constant<int, 1>;
+        using M2 = std::integral_constant<int, 2>;
 
         int4 next_it = make_int4(0, 0, 0, 0);
         if ((int)blockIdx.x < n_work) next_it = load_item(p, blockIdx.x);
@@ -702,19 +704,20 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             if (n_t == 0) continue;  // this tile has no rows in this block
             m_used = 0.f;
             l_run = 0.f;
+            // The last two steps are the diagonal tile: key 64 b + c is masked for query row r when
+            // 64 b + c > r.  Per warp (32 rows) a 64-key half is untouched (rows 64-127, b = 0),
+            // partly masked (rows 0-63, b = 0; rows 64-127, b = 1) or masked altogether (rows 0-63,
+            // b = 1).
             for (int j = 0; j + 1 < n_t; ++j) {
-                step(B0{}, B0{}, j == 0);
-                step(B1{}, B0{}, false);
+                step(M0{}, 0, j == 0);
+                step(M0{}, 1, false);
                 ph_s ^= 1;
             }
-            // diagonal tile: key 64 b + c is masked for query row r when 64 b + c > r.  Per warp
-            // (32 rows) a 64-key half is either untouched, partly masked or masked altogether.
-            if (wq >= 2) {
-                step(B0{}, B0{}, n_t == 1);
-                step(B1{}, B1{}, false);
-            } else {
-                step(B0{}, B1{}, n_t == 1);
-                step(B1{}, B2{}, false);
+            for (int b = 0; b < 2; ++b) {
+                if (b == 1 && wq < 2)
+                    step(M2{}, b, false);
+                else
+                    step(M1{}, b, b == 0 && n_t == 1);  // (masks nothing for rows 64-127, b = 0)
             }
             ph_s ^= 1;
             // ---- hand the row's (m, l) to the epilogue warps and go on to the next item -----------
