@@ -355,7 +355,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                     const int row_g = k.row0 + t * BM + row;
                     const float inv_l = 1.f / ml.y;
                     __nv_bfloat16* orow = p.o + ((k.t0 + row_g) * p.Hq + k.h) * (int64_t)D;
-#pragma unroll
+#pragma unroll 2
                     for (int c = 0; c < D / 16; ++c) {
                         uint32_t r[16];
                         ptx::tmem_ld16(tO + c * 16, r);
@@ -637,15 +637,15 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                         const float alpha = need ? ex2_approx(m_used - m_new) : 1.f;
                         if (need) m_used = m_new;
                         l_run *= alpha;
-#pragma unroll
-                        for (int c = 0; c < D / 32; ++c) {
-                            uint32_t r[32];
-                            ptx::tmem_ld32(tO + c * 32, r);
+#pragma unroll 1  // rare: keep it small (instruction cache)
+                        for (int c = 0; c < D / 16; ++c) {
+                            uint32_t r[16];
+                            ptx::tmem_ld16(tO + c * 16, r);
                             ptx::tmem_wait_ld();
 #pragma unroll
-                            for (int i = 0; i < 32; ++i)
+                            for (int i = 0; i < 16; ++i)
                                 r[i] = __float_as_uint(__uint_as_float(r[i]) * alpha);
-                            ptx::tmem_st32(tO + c * 32, r);
+                            ptx::tmem_st16(tO + c * 16, r);
                         }
                     }
                 }
