@@ -180,6 +180,7 @@ struct AttnParams {
     int64_t T;
     int Hq, Hkv;
     float scale_log2;  // |softmax_scale| * log2(e); a negative scale negates Q inside the MMA
+    float inv_group;   // 1 / (Hq / Hkv)
     int o_align32;     // o is 32-byte aligned: the epilogue may use 256-bit stores
 };
 
@@ -218,28 +219,47 @@ struct Work {
     int64_t t0;      // first token of the sequence
     int L;           // sequence length
     int row0;        // first row of the block inside the sequence
-    int n[2];        // KV tiles of tile 0 / tile 1 (0 = tile has no rows)
+    int n0, n1;      // KV tiles of tile 0 / tile 1 (0 = tile has no rows)
     int n_kv;        // max of the two
+    __device__ __forceinline__ int n(int t) const { return t ? n1 : n0; }
 };
 
-// The descriptor of work unit w is loaded one unit ahead and decoded only when the unit starts:
-// the load (an L2 round trip) is then hidden behind the unit before it.
-__device__ __forceinline__ int4 load_item(const AttnParams& p, int w) {
-    return __ldg(p.items + w / p.Hq);
-}
-__device__ __forceinline__ Work decode_work(const AttnParams& p, int w, const int4 it) {
-    Work k;
-    const int item = w / p.Hq;
-    k.h = w - item * p.Hq;
-    k.g = k.h / (p.Hq / p.Hkv);
-    k.t0 = it.x;
-    k.L = it.y;
-    k.row0 = it.z * BQ;
-    k.n[0] = 2 * it.z + 1;
-    k.n[1] = (k.row0 + BM < k.L) ? 2 * it.z + 2 : 0;
-    k.n_kv = max(k.n[0], k.n[1]);
-    return k;
-}
+// The work units of one CTA: w = blockIdx.x, + gridDim.x, ...; unit w is q head w % Hq of entry
+// w / Hq of the work list.  (entry, head) are stepped, not divided out, and the descriptor of a
+// unit is loaded one unit ahead and decoded only when the unit starts, so the load (an L2 round
+// trip) hides behind the unit before it.
+struct WorkCursor {
+    int item, h, d_item, d_h;
+    int4 it;
+    __device__ __forceinline__ WorkCursor(const AttnParams& p, int n_work) {
+        item = (int)blockIdx.x / p.Hq;
+        h = (int)blockIdx.x - item * p.Hq;
+        d_item = (int)gridDim.x / p.Hq;
+        d_h = (int)gridDim.x - d_item * p.Hq;
+        it = make_int4(0, 0, 0, 0);
+        if ((int)blockIdx.x < n_work) it = __ldg(p.items + item);
+    }
+    // the current unit; `more`: there is a next one (its descriptor is requested now)
+    __device__ __forceinline__ Work take(const AttnParams& p, bool more) {
+        Work k;
+        k.h = h;
+        k.g = __float2int_rd(((float)h + 0.5f) * p.inv_group);  // h / (Hq / Hkv)
+        k.t0 = it.x;
+        k.L = it.y;
+        k.row0 = it.z * BQ;
+        k.n0 = 2 * it.z + 1;
+        k.n1 = (k.row0 + BM < k.L) ? 2 * it.z + 2 : 0;
+        k.n_kv = max(k.n0, k.n1);
+        item += d_item;
+        h += d_h;
+        if (h >= p.Hq) {
+            h -= p.Hq;
+            ++item;
+        }
+        if (more) it = __ldg(p.items + item);
+        return k;
+    }
+};
 
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;
@@ -338,14 +358,12 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
             const float2* stat = reinterpret_cast<const float2*>(smem + SL::kStat);
             uint32_t ph[2] = {0, 0};
-            int4 next_it = make_int4(0, 0, 0, 0);
-            if ((int)blockIdx.x < n_work) next_it = load_item(p, blockIdx.x);
+            WorkCursor cursor(p, n_work);
             for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-                const Work k = decode_work(p, w, next_it);
-                if (w + (int)gridDim.x < n_work) next_it = load_item(p, w + gridDim.x);
+                const Work k = cursor.take(p, w + (int)gridDim.x < n_work);
 #pragma unroll 1
                 for (int t = 0; t < 2; ++t) {
-                    if (k.n[t] == 0) continue;
+                    if (k.n(t) == 0) continue;
                     ptx::mbar_wait(bar(kBarStat, t), ph[t]);   // the softmax group is done with the item
                     ptx::mbar_wait(bar(kBarODone, t), ph[t]);  // ... and so is the last PV_t
                     ph[t] ^= 1;
@@ -395,11 +413,9 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         } else if (warp == kWarpProducer) {
             // ================================ TMA producer ================================
             uint32_t pos = 0, ph_q[2] = {0, 0};
-            int4 next_it = make_int4(0, 0, 0, 0);
-            if ((int)blockIdx.x < n_work) next_it = load_item(p, blockIdx.x);
+            WorkCursor cursor(p, n_work);
             for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-                const Work k = decode_work(p, w, next_it);
-                if (w + (int)gridDim.x < n_work) next_it = load_item(p, w + gridDim.x);
+                const Work k = cursor.take(p, w + (int)gridDim.x < n_work);
                 auto load_q = [&](int t) {
                     ptx::mbar_wait(bar(kBarQEmpty, t), ph_q[t] ^ 1);
                     ph_q[t] ^= 1;
@@ -430,7 +446,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                 };
                 load_q(0);
                 load_kv(&tm_k, 0);
-                if (k.n[1]) load_q(1);
+                if (k.n1) load_q(1);
                 load_kv(&tm_v, 0);
                 for (int j = 1; j < k.n_kv; ++j) {
                     load_kv(&tm_k, j);
@@ -496,12 +512,10 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             // so S(u+2) overwrites P(u) right behind PV(u) in the (in-order) tensor pipe and is
             // ready, as a rule, before the softmax group has finished step u + 1.
             uint32_t pos = 0, ph_q = 0, ph_p = 0, ph_f = 0;
-            int4 next_it = make_int4(0, 0, 0, 0);
-            if ((int)blockIdx.x < n_work) next_it = load_item(p, blockIdx.x);
+            WorkCursor cursor(p, n_work);
             for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-                const Work k = decode_work(p, w, next_it);
-                if (w + (int)gridDim.x < n_work) next_it = load_item(p, w + gridDim.x);
-                const int n_t = k.n[t];
+                const Work k = cursor.take(p, w + (int)gridDim.x < n_work);
+                const int n_t = k.n(t);
                 const uint32_t base = pos;
                 if (n_t > 0) {
                     ptx::mbar_wait(bar(kBarQFull, t), ph_q);
@@ -695,12 +709,10 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         using M1 = std::integral_constant<int, 1>;
         using M2 = std::integral_constant<int, 2>;
 
-        int4 next_it = make_int4(0, 0, 0, 0);
-        if ((int)blockIdx.x < n_work) next_it = load_item(p, blockIdx.x);
+        WorkCursor cursor(p, n_work);
         for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-            const Work k = decode_work(p, w, next_it);
-            if (w + (int)gridDim.x < n_work) next_it = load_item(p, w + gridDim.x);
-            const int n_t = k.n[t];
+            const Work k = cursor.take(p, w + (int)gridDim.x < n_work);
+            const int n_t = k.n(t);
             if (n_t == 0) continue;  // this tile has no rows in this block
             m_used = 0.f;
             l_run = 0.f;
@@ -842,6 +854,7 @@ extern "C" mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k,
     p.Hq = Hq;
     p.Hkv = Hkv;
     p.scale_log2 = fabsf(softmax_scale) * kLog2e;
+    p.inv_group = 1.0f / (float)(Hq / Hkv);
     p.o_align32 = (reinterpret_cast<uintptr_t>(o) & 31u) == 0 ? 1 : 0;
     const int negate_q = softmax_scale < 0.f ? 1 : 0;
     const int64_t max_work = (total_tokens / BQ + n_seqs) * (int64_t)Hq;
