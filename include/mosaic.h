@@ -150,6 +150,9 @@ mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k, const void
  * inputs to the device, runs mosaic_gate_compact, reads S / total_tokens / max_seqlen back,
  * copies the survivors' packed Q/K/V to the device, runs mosaic_agg_prefill_attn and copies every
  * result back.  SYNCHRONOUS: returns after the results are in the host buffers.
+ * The survivors' Q/K/V go up, through the attention kernel and back in chunks of whole sequences on
+ * two internal copy streams (created on first use, one set per process), so the two PCIe
+ * directions and the kernel overlap; concurrent calls from several threads serialise.
  *
  *   answers_h, expert_conf_h, ctx_len_h  [host] as mosaic_gate / mosaic_compact.
  *   mode_h, conf_h, bypass_h             [host] [Q] outputs (mode_h, conf_h may be NULL).

@@ -1,8 +1,13 @@
 // stage.cu -- mosaic_stage_host: the whole confidence-gated aggregator stage (Alg. 1)
 // from HOST buffers: H2D copies, gate + compaction, survivors' prefill attention, D2H copies.
 // Only marshalling lives here; every step of the path runs in the kernels of gate.cu / attn.cu.
+// The survivors go through in chunks of whole sequences: chunk c+1 is on its way to the device
+// and the results of chunk c-1 on their way back while chunk c is in the attention kernel (PCIe
+// is full duplex, and at 2.6 GB per C2 step the copies are 94 % of the call).
 #include <cuda_runtime.h>
 #include <stdint.h>
+
+#include <mutex>
 
 #include "common.cuh"
 
@@ -64,6 +69,37 @@ Arena carve_arena(void* base, int64_t Q, int32_t E, int64_t T_cap, int32_t Hq, i
     a.attn_ws = take(a.attn_ws_bytes);
     a.total = off;
     return a;
+}
+
+// Copy streams and events of the chunk pipeline (one set per process; the call is synchronous,
+// so one call uses them at a time -- concurrent calls serialise on the mutex).
+constexpr int kMaxChunks = 16;
+struct Pipe {
+    cudaStream_t in = nullptr, out = nullptr;
+    cudaEvent_t ev_in[kMaxChunks], ev_out[kMaxChunks], ev_ready;
+    int device = -1;
+    bool ok = false;
+    std::mutex mu;
+};
+Pipe& pipe() {
+    static Pipe p;
+    return p;
+}
+bool pipe_init(Pipe& p) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return false;
+    if (p.ok && p.device == dev) return true;
+    if (p.ok) return false;  // one device per process (one process per GPU)
+    if (cudaStreamCreateWithFlags(&p.in, cudaStreamNonBlocking) != cudaSuccess) return false;
+    if (cudaStreamCreateWithFlags(&p.out, cudaStreamNonBlocking) != cudaSuccess) return false;
+    for (int i = 0; i < kMaxChunks; ++i) {
+        if (cudaEventCreateWithFlags(&p.ev_in[i], cudaEventDisableTiming) != cudaSuccess) return false;
+        if (cudaEventCreateWithFlags(&p.ev_out[i], cudaEventDisableTiming) != cudaSuccess) return false;
+    }
+    if (cudaEventCreateWithFlags(&p.ev_ready, cudaEventDisableTiming) != cudaSuccess) return false;
+    p.device = dev;
+    p.ok = true;
+    return true;
 }
 
 }  // namespace
@@ -137,14 +173,58 @@ extern "C" mosaic_status_t mosaic_stage_host(
     if (T == 0) return MOSAIC_OK;
     if (T > T_cap) return MOSAIC_ERR_WORKSPACE_TOO_SMALL;
     if (!q_h || !k_h || !v_h || !o_h || !lse_h) return MOSAIC_ERR_INVALID_ARG;
-    MOSAIC_CUDA_TRY(cudaMemcpyAsync(a.q, q_h, (size_t)T * Hq * D * 2, H2D, s));
-    MOSAIC_CUDA_TRY(cudaMemcpyAsync(a.k, k_h, (size_t)T * Hkv * D * 2, H2D, s));
-    MOSAIC_CUDA_TRY(cudaMemcpyAsync(a.v, v_h, (size_t)T * Hkv * D * 2, H2D, s));
-    st = mosaic_agg_prefill_attn(a.q, a.k, a.v, a.cu_seqlens, (int32_t)n_att, T, sc.max_len, Hq,
-                                 Hkv, D, softmax_scale, a.o, a.lse, a.attn_ws, a.attn_ws_bytes, s);
-    if (st != MOSAIC_OK) return st;
-    MOSAIC_CUDA_TRY(cudaMemcpyAsync(o_h, a.o, (size_t)T * Hq * D * 2, D2H, s));
-    MOSAIC_CUDA_TRY(cudaMemcpyAsync(lse_h, a.lse, (size_t)T * Hq * 4, D2H, s));
+    // Chunks of whole sequences of about T / n_chunks tokens each (at least ~16 k tokens a chunk:
+    // smaller ones would make the attention launches and the copies latency-bound).
+    Pipe& pp = pipe();
+    std::lock_guard<std::mutex> lock(pp.mu);
+    if (!pipe_init(pp)) return MOSAIC_ERR_CUDA;
+    int n_chunks = (int)(T / 16384);
+    n_chunks = n_chunks < 1 ? 1 : (n_chunks > kMaxChunks ? kMaxChunks : n_chunks);
+    int64_t first[kMaxChunks + 1];  // first sequence of every chunk
+    {
+        int c = 0;
+        first[0] = 0;
+        for (int64_t q = 0; q < n_att && c + 1 < n_chunks; ++q)
+            if (cu_seqlens_h[q + 1] >= (T * (c + 1)) / n_chunks) first[++c] = q + 1;
+        n_chunks = c + 1;
+        first[n_chunks] = n_att;
+    }
+    // the copy streams start after everything this call has enqueued on s so far
+    MOSAIC_CUDA_TRY(cudaEventRecord(pp.ev_ready, s));
+    MOSAIC_CUDA_TRY(cudaStreamWaitEvent(pp.in, pp.ev_ready, 0));
+    MOSAIC_CUDA_TRY(cudaStreamWaitEvent(pp.out, pp.ev_ready, 0));
+    const size_t q_row = (size_t)Hq * D * 2, kv_row = (size_t)Hkv * D * 2;
+    for (int c = 0; c < n_chunks; ++c) {
+        const int64_t s0 = first[c], s1 = first[c + 1];
+        const int64_t t0 = cu_seqlens_h[s0], t1 = cu_seqlens_h[s1];
+        if (s1 == s0 || t1 == t0) continue;
+        const size_t rows = (size_t)(t1 - t0);
+        auto at = [](const void* base, size_t off) { return static_cast<const char*>(base) + off; };
+        auto at_w = [](void* base, size_t off) { return static_cast<char*>(base) + off; };
+        MOSAIC_CUDA_TRY(cudaMemcpyAsync(at_w(a.q, t0 * q_row), at(q_h, t0 * q_row), rows * q_row, H2D, pp.in));
+        MOSAIC_CUDA_TRY(cudaMemcpyAsync(at_w(a.k, t0 * kv_row), at(k_h, t0 * kv_row), rows * kv_row, H2D, pp.in));
+        MOSAIC_CUDA_TRY(cudaMemcpyAsync(at_w(a.v, t0 * kv_row), at(v_h, t0 * kv_row), rows * kv_row, H2D, pp.in));
+        MOSAIC_CUDA_TRY(cudaEventRecord(pp.ev_in[c], pp.in));
+        MOSAIC_CUDA_TRY(cudaStreamWaitEvent(s, pp.ev_in[c], 0));
+        // the sequences s0 .. s1-1 of the same packed buffers: cu_seqlens holds absolute offsets
+        st = mosaic_agg_prefill_attn(a.q, a.k, a.v, a.cu_seqlens + s0, (int32_t)(s1 - s0), T,
+                                     sc.max_len, Hq, Hkv, D, softmax_scale, a.o, a.lse, a.attn_ws,
+                                     a.attn_ws_bytes, s);
+        if (st != MOSAIC_OK) {
+            cudaStreamSynchronize(pp.in);
+            cudaStreamSynchronize(s);
+            cudaStreamSynchronize(pp.out);
+            return st;
+        }
+        MOSAIC_CUDA_TRY(cudaEventRecord(pp.ev_out[c], s));
+        MOSAIC_CUDA_TRY(cudaStreamWaitEvent(pp.out, pp.ev_out[c], 0));
+        MOSAIC_CUDA_TRY(cudaMemcpyAsync(at_w(o_h, t0 * q_row), at(a.o, t0 * q_row), rows * q_row, D2H, pp.out));
+        // LSE is [Hq, T]: the chunk's columns of every head
+        MOSAIC_CUDA_TRY(cudaMemcpy2DAsync(lse_h + t0, (size_t)T * 4, a.lse + t0, (size_t)T * 4,
+                                          rows * 4, (size_t)Hq, D2H, pp.out));
+    }
+    MOSAIC_CUDA_TRY(cudaStreamSynchronize(pp.in));
     MOSAIC_CUDA_TRY(cudaStreamSynchronize(s));
+    MOSAIC_CUDA_TRY(cudaStreamSynchronize(pp.out));
     return MOSAIC_OK;
 }

@@ -208,3 +208,30 @@ def test_stage_host_matches_oracle():
     O_ref, lse_ref = oracle.attn_full(P.bf16_bits(q), P.bf16_bits(k), P.bf16_bits(v), cu, scale)
     assert np.abs(r["o"][:T].float().numpy() - O_ref).max() <= P.O_TOL
     assert np.abs(r["lse"][:cfg.Hq * T].view(cfg.Hq, T).numpy() - lse_ref).max() <= P.LSE_TOL
+
+
+def test_stage_host_chunked_matches_oracle():
+    """mosaic_stage_host on the bench config: ~159 k tokens go through in 9 chunks of whole
+    sequences over the copy streams; gate outputs bit-exact, sampled attention rows (every
+    sequence's tile and sequence edges, hence every chunk) against the oracle."""
+    from paper_2606_03014_b200 import mosaic
+    cfg = wl.C2
+    gi = wl.gate_inputs(cfg, 0)
+    want = P.oracle_gate_compact(gi, 0)
+    cu = want["cu_seqlens"]
+    T = int(cu[-1])
+    assert T > 8 * 16384
+    q, k, v = wl.qkv(cfg, 0, T)
+    scale = wl.softmax_scale(cfg)
+    r = mosaic.stage_host(torch.from_numpy(gi.answers), None, torch.from_numpy(gi.ctx_len), gi.tau,
+                          0, q, k, v, scale)
+    S = int(r["n_survivors"])
+    assert S == want["n_survivors"] and int(r["total_tokens"]) == T
+    assert np.array_equal(r["bypass"].numpy(), want["bypass"])
+    assert np.array_equal(r["survivor_idx"][:S].numpy(), want["survivor_idx"])
+    assert np.array_equal(r["cu_seqlens"][:S + 1].numpy(), cu)
+    rs, rh, rp = wl.sample_rows(cu, cfg.Hq, cfg.Hkv, 0, cfg.config_id, n_random=256)
+    o = r["o"][:T]
+    lse = r["lse"][:cfg.Hq * T].view(cfg.Hq, T)
+    eo, el = P.check_attn_rows(o, lse, q, k, v, cu, rs, rh, rp, scale)
+    assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
