@@ -73,7 +73,13 @@ Arena carve_arena(void* base, int64_t Q, int32_t E, int64_t T_cap, int32_t Hq, i
 
 // Copy streams and events of the chunk pipeline (one set per process; the call is synchronous,
 // so one call uses them at a time -- concurrent calls serialise on the mutex).
-constexpr int kMaxChunks = 16;
+#ifndef MOSAIC_STAGE_CHUNK_TOKENS
+#define MOSAIC_STAGE_CHUNK_TOKENS 8192
+#endif
+#ifndef MOSAIC_STAGE_MAX_CHUNKS
+#define MOSAIC_STAGE_MAX_CHUNKS 16
+#endif
+constexpr int kMaxChunks = MOSAIC_STAGE_MAX_CHUNKS;
 struct Pipe {
     cudaStream_t in = nullptr, out = nullptr;
     cudaEvent_t ev_in[kMaxChunks], ev_out[kMaxChunks], ev_ready;
@@ -173,12 +179,12 @@ extern "C" mosaic_status_t mosaic_stage_host(
     if (T == 0) return MOSAIC_OK;
     if (T > T_cap) return MOSAIC_ERR_WORKSPACE_TOO_SMALL;
     if (!q_h || !k_h || !v_h || !o_h || !lse_h) return MOSAIC_ERR_INVALID_ARG;
-    // Chunks of whole sequences of about T / n_chunks tokens each (at least ~16 k tokens a chunk:
+    // Chunks of whole sequences of about T / n_chunks tokens each (at least ~8 k tokens a chunk:
     // smaller ones would make the attention launches and the copies latency-bound).
     Pipe& pp = pipe();
     std::lock_guard<std::mutex> lock(pp.mu);
     if (!pipe_init(pp)) return MOSAIC_ERR_CUDA;
-    int n_chunks = (int)(T / 16384);
+    int n_chunks = (int)(T / MOSAIC_STAGE_CHUNK_TOKENS);
     n_chunks = n_chunks < 1 ? 1 : (n_chunks > kMaxChunks ? kMaxChunks : n_chunks);
     int64_t first[kMaxChunks + 1];  // first sequence of every chunk
     {

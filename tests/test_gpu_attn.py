@@ -211,7 +211,7 @@ def test_stage_host_matches_oracle():
 
 
 def test_stage_host_chunked_matches_oracle():
-    """mosaic_stage_host on the bench config: ~159 k tokens go through in 9 chunks of whole
+    """mosaic_stage_host on the bench config: ~159 k tokens go through in 16 chunks of whole
     sequences over the copy streams; gate outputs bit-exact, sampled attention rows (every
     sequence's tile and sequence edges, hence every chunk) against the oracle."""
     from paper_2606_03014_b200 import mosaic
