@@ -115,6 +115,44 @@ def compact(bypass, ctx_len):
                 total_tokens=int(tot[0]), max_seqlen=int(mx[0]))
 
 
+def assemble_context(survivor_idx, cu_seqlens, prompt_tokens, prompt_off, trace_tokens, trace_off,
+                     E: int):
+    """the survivors' aggregator contexts as one packed token batch.  The
+    aggregator reads "the combined output or reasoning traces of its experts" (Alg. 1
+    `Aggregator(q, {a_i})`); reading N1-1 fixes the order the paper leaves open:
+    context of survivor j (question q = survivor_idx[j]) = prompt(q) ++ trace(q,0) ++ ... ++
+    trace(q,E-1).  Written out sequence by sequence, segment by segment (plain slices, no
+    arithmetic to get wrong beyond the offsets).  A sequence whose cu_seqlens length differs from
+    prompt + traces is truncated, or padded with -1, and counted in n_mismatch.
+
+    Returns dict(input_ids int32 [T], position_ids int32 [T], n_mismatch int).
+    """
+    idx = _c(survivor_idx, np.int32)
+    cu = _c(cu_seqlens, np.int64)
+    pt, po = _c(prompt_tokens, np.int32), _c(prompt_off, np.int64)
+    tt, to = _c(trace_tokens, np.int32), _c(trace_off, np.int64)
+    S = idx.shape[0]
+    assert cu.shape == (S + 1,)
+    T = int(cu[S]) if S else 0
+    ids = np.full(T, -1, np.int32)
+    pos = np.empty(T, np.int32)
+    n_mismatch = 0
+    for j in range(S):
+        q = int(idx[j])
+        parts = [pt[po[q]:po[q + 1]]]
+        for e in range(E):
+            parts.append(tt[to[q * E + e]:to[q * E + e + 1]])
+        seq = np.concatenate(parts) if parts else np.empty(0, np.int32)
+        a, b = int(cu[j]), int(cu[j + 1])
+        L = b - a
+        if seq.shape[0] != L:
+            n_mismatch += 1
+        m = min(L, seq.shape[0])
+        ids[a:a + m] = seq[:m]
+        pos[a:b] = np.arange(L, dtype=np.int32)
+    return dict(input_ids=ids, position_ids=pos, n_mismatch=n_mismatch)
+
+
 def _check_qkv(q, k, v, cu_seqlens):
     q = _c(q, np.uint16)
     k = _c(k, np.uint16)

@@ -105,6 +105,33 @@ def ctx_len(cfg: Config, seed: int, Q: Optional[int] = None):
     return n.astype(np.int32)
 
 
+_A_PARTS, _A_TOKENS = 21, 22
+VOCAB = 151936  # the aggregator models the paper runs are Qwen-family; any vocabulary would do
+
+
+def context_parts(cfg: Config, seed: int, Q: Optional[int] = None, E: Optional[int] = None):
+    """SURVEY 8(f) N1 inputs: every question's context split into a prompt and E expert traces
+    whose lengths add up to ctx_len(cfg, seed)[q] (so cu_seqlens is the one every other step sees).
+    The prompt is min(256, n // 4) tokens, as in the ctx recipes of configs 2-3; E - 1 seeded cut
+    points split the rest (a trace may be empty).  Returns (prompt_tokens int32, prompt_off int64
+    [Q+1], trace_tokens int32, trace_off int64 [Q*E+1]) with seeded token ids in [0, VOCAB)."""
+    Q = cfg.Q if Q is None else Q
+    E = cfg.E if E is None else E
+    n = ctx_len(cfg, seed, Q).astype(np.int64)
+    g = rng(seed, cfg.config_id, _A_PARTS)
+    p_len = np.minimum(256, n // 4)
+    rest = n - p_len
+    cuts = np.sort((g.random((Q, max(E - 1, 0))) * (rest[:, None] + 1)).astype(np.int64), axis=1)
+    edges = np.concatenate([np.zeros((Q, 1), np.int64), cuts, rest[:, None]], axis=1)
+    t_len = np.diff(edges, axis=1)  # [Q, E]
+    prompt_off = np.concatenate([[0], np.cumsum(p_len)]).astype(np.int64)
+    trace_off = np.concatenate([[0], np.cumsum(t_len.reshape(-1))]).astype(np.int64)
+    gt = rng(seed, cfg.config_id, _A_TOKENS)
+    prompt_tokens = gt.integers(0, VOCAB, size=int(prompt_off[-1]), dtype=np.int32)
+    trace_tokens = gt.integers(0, VOCAB, size=int(trace_off[-1]), dtype=np.int32)
+    return prompt_tokens, prompt_off, trace_tokens, trace_off
+
+
 @dataclass
 class GateInputs:
     answers: np.ndarray
