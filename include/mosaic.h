@@ -146,6 +146,32 @@ mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k, const void
                                         void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * mosaic_assemble_context -- SURVEY.md section 8(f) N1 (a "next" row, between G5 and A1): the
+ * survivors' aggregator contexts as one packed token batch.  The aggregator "process[es] the
+ * combined output or reasoning traces of its experts" (Alg. 1
+ * `Aggregator(q, {a_i})`); template and order are not given, reading N1-1 fixes
+ * them: the context of survivor j (question q = survivor_idx[j]) is
+ *     prompt(q) ++ trace(q, 0) ++ trace(q, 1) ++ ... ++ trace(q, E-1).
+ *
+ *   survivor_idx  [dev] int32 [n_survivors], cu_seqlens [dev] int64 [n_survivors + 1]: as written
+ *                 by mosaic_compact (ctx_len[q] = tokens of q's context).
+ *   n_survivors, max_seqlen  host values read back from mosaic_compact.
+ *   prompt_tokens [dev] int32, the prompts of all Q questions packed; prompt_off [dev] int64 [Q+1].
+ *   trace_tokens  [dev] int32, the traces packed in (q, e) order; trace_off [dev] int64 [Q*E + 1].
+ *   input_ids     [dev] int32 [total_tokens]  out: the packed contexts.
+ *   position_ids  [dev] int32 [total_tokens]  out: 0, 1, ... inside every sequence.
+ *   n_mismatch    [dev] int32 or NULL         out: sequences whose cu_seqlens length differs from
+ *                 prompt + traces; such a sequence is truncated, or padded with -1.
+ * Nothing is owned or retained; asynchronous on cuda_stream.  1 <= E <= MOSAIC_MAX_EXPERTS.
+ * ------------------------------------------------------------------------------------------- */
+mosaic_status_t mosaic_assemble_context(const int32_t* survivor_idx, const int64_t* cu_seqlens,
+                                        int32_t n_survivors, int32_t max_seqlen,
+                                        const int32_t* prompt_tokens, const int64_t* prompt_off,
+                                        const int32_t* trace_tokens, const int64_t* trace_off,
+                                        int32_t E, int32_t* input_ids, int32_t* position_ids,
+                                        int32_t* n_mismatch, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * mosaic_stage_host -- the whole stage from HOST buffers (the end-to-end call): copies the gate
  * inputs to the device, runs mosaic_gate_compact, reads S / total_tokens / max_seqlen back,
  * copies the survivors' packed Q/K/V to the device, runs mosaic_agg_prefill_attn and copies every

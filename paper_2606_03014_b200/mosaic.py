@@ -30,6 +30,8 @@ SIGNATURES = {
     "mosaic_agg_prefill_attn_workspace_bytes": (_sz, [_i32, _i64, _i32, _i32, _i32]),
     "mosaic_agg_prefill_attn": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i64, _i32, _i32, _i32,
                                                _i32, _f32, _vp, _vp, _vp, _sz, _vp]),
+    "mosaic_assemble_context": (ctypes.c_int, [_vp, _vp, _i32, _i32, _vp, _vp, _vp, _vp, _i32, _vp,
+                                               _vp, _vp, _vp]),
     "mosaic_stage_host_arena_bytes": (_sz, [_i64, _i32, _i64, _i32, _i32, _i32]),
     "mosaic_stage_host": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _f32, _i32, _vp, _vp, _vp, _vp,
                                          _vp, _vp, _vp, _vp, _i32, _vp, _vp, _vp, _i64, _i32, _i32,
@@ -195,6 +197,29 @@ def agg_prefill_attn(q, k, v, cu_seqlens, n_seqs, max_seqlen, softmax_scale, *, 
         _dptr(workspace), workspace.numel(), _stream(stream))
     _check("mosaic_agg_prefill_attn", st)
     return o, lse
+
+
+def assemble_context(survivor_idx, cu_seqlens, n_survivors, max_seqlen, total_tokens,
+                     prompt_tokens, prompt_off, trace_tokens, trace_off, E, *, input_ids=None,
+                     position_ids=None, n_mismatch=None, stream=None):
+    """mosaic_assemble_context.  All tensors on the device; returns
+    (input_ids int32 [total_tokens], position_ids int32 [total_tokens], n_mismatch int32 [1])."""
+    dev = cu_seqlens.device
+    if input_ids is None:
+        input_ids = torch.empty(max(int(total_tokens), 1), dtype=torch.int32, device=dev)
+    if position_ids is None:
+        position_ids = torch.empty(max(int(total_tokens), 1), dtype=torch.int32, device=dev)
+    if n_mismatch is None:
+        n_mismatch = torch.empty(1, dtype=torch.int32, device=dev)
+    st = load().mosaic_assemble_context(
+        _dptr(survivor_idx, torch.int32, "survivor_idx"), _dptr(cu_seqlens, torch.int64, "cu_seqlens"),
+        int(n_survivors), int(max_seqlen), _dptr(prompt_tokens, torch.int32, "prompt_tokens"),
+        _dptr(prompt_off, torch.int64, "prompt_off"), _dptr(trace_tokens, torch.int32, "trace_tokens"),
+        _dptr(trace_off, torch.int64, "trace_off"), int(E), _dptr(input_ids, torch.int32, "input_ids"),
+        _dptr(position_ids, torch.int32, "position_ids"), _dptr(n_mismatch, torch.int32, "n_mismatch"),
+        _stream(stream))
+    _check("mosaic_assemble_context", st)
+    return input_ids[:int(total_tokens)], position_ids[:int(total_tokens)], n_mismatch
 
 
 def stage_host_arena_bytes(Q, E, T_cap, Hq, Hkv, D) -> int:
