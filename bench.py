@@ -288,6 +288,52 @@ def bench_gate_q24(torch, mosaic, pk):
             "achieved_gbs": byts / t / 1e9, "frac_of_measured_hbm": byts / t / 1e9 / pk["hbm_gbs"]}
 
 
+def bench_assemble(torch, mosaic, pk):
+    """SURVEY 8(f) N1 (a "next" row): mosaic_assemble_context over 2048 survivors of the C5 context
+    recipe (U{8192..32768} tokens each, E = 8, prompt 256 + 8 traces at seeded cut points).
+    Algorithmic bytes: 4 read + 8 written per token.  Parity: tests/test_gpu_assemble.py."""
+    S, E = 2048, 8
+    g = np.random.default_rng(31)
+    n = g.integers(8192, 32769, size=S).astype(np.int64)
+    p_len = np.full(S, 256, np.int64)
+    cuts = np.sort((g.random((S, E - 1)) * (n - 256 + 1)[:, None]).astype(np.int64), axis=1)
+    edges = np.concatenate([np.zeros((S, 1), np.int64), cuts, (n - 256)[:, None]], axis=1)
+    t_len = np.diff(edges, axis=1)
+    po = np.concatenate([[0], np.cumsum(p_len)]).astype(np.int64)
+    to = np.concatenate([[0], np.cumsum(t_len.reshape(-1))]).astype(np.int64)
+    cu = np.concatenate([[0], np.cumsum(n)]).astype(np.int64)
+    T = int(cu[-1])
+    dev = "cuda"
+    gt = torch.Generator(device=dev).manual_seed(31)
+    pt = torch.randint(0, 151936, (int(po[-1]),), device=dev, generator=gt, dtype=torch.int32)
+    tt = torch.randint(0, 151936, (int(to[-1]),), device=dev, generator=gt, dtype=torch.int32)
+    idx = torch.arange(S, device=dev, dtype=torch.int32)
+    cu_d, po_d, to_d = (torch.from_numpy(x).to(dev) for x in (cu, po, to))
+    ids = torch.empty(T, dtype=torch.int32, device=dev)
+    pos = torch.empty(T, dtype=torch.int32, device=dev)
+    mm = torch.empty(1, dtype=torch.int32, device=dev)
+    call = lambda: mosaic.assemble_context(idx, cu_d, S, int(n.max()), T, pt, po_d, tt, to_d, E,
+                                           input_ids=ids, position_ids=pos, n_mismatch=mm)
+    for _ in range(2):
+        call()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in range(5)]
+    torch.cuda.synchronize()
+    for e0, e1 in evs:   # 0.5 GB per call: every call is L2-cold
+        e0.record()
+        call()
+        e1.record()
+    torch.cuda.synchronize()
+    assert int(mm.item()) == 0
+    t = float(np.mean([e0.elapsed_time(e1) for e0, e1 in evs])) * 1e-3
+    byts = 12.0 * T
+    return {"workload": "SURVEY 8(f) N1: 2048 contexts of U{8192..32768} tokens, E=8", "tokens": T,
+            "us_per_call": t * 1e6, "gtokens_per_s": T / t / 1e9,
+            "roofline": {"bound": "hbm", "achieved": byts / t / 1e9, "peak": pk["hbm_gbs"],
+                         "unit": "GB/s", "frac": byts / t / 1e9 / pk["hbm_gbs"], "traffic": None,
+                         "algorithmic_bytes": byts}}
+
+
 def run_product(args):
     import torch
     import torch.distributed as dist
@@ -396,6 +442,7 @@ def run_product(args):
         return
     gate_info = bench_gate_c5(torch, mosaic, wl, pk, steps=40, warmup=8)
     gate_info["q24"] = bench_gate_q24(torch, mosaic, pk)
+    assemble_info = bench_assemble(torch, mosaic, pk)
     f, t, threads, desc = oracle_sample(cfg, 0, args.cpu_rows)
     attn_tflops = flops / (attn_ms * 1e-3) / 1e12
     traffic = None
@@ -419,6 +466,7 @@ def run_product(args):
                      "traffic": traffic, "kernel": "attn_fwd (+ schedule_kernel)",
                      "ms_per_launch": attn_ms, "peak_kind": "burst bf16_tflops"},
         "gate": gate_info,
+        "assemble": assemble_info,
         "cpu_baseline": {"value": f / t / 1e12, "unit": UNIT, "cores": threads, "kind": "oracle",
                          "sample": desc},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
