@@ -84,15 +84,26 @@ __global__ void __launch_bounds__(kAsmThreads) assemble_kernel(const AssembleArg
     //  153 against 132 us on the bench workload.)
     const int64_t base = (t0 + i0) & ~int64_t(3);
     const int64_t n_groups = (t0 + i1 - base + 3) >> 2;
+#pragma unroll 2
     for (int64_t k = threadIdx.x; k < n_groups; k += kAsmThreads) {
         const int64_t o = base + 4 * k;  // output element of the group's first token
         const int64_t i = o - t0;        // its index in the sequence (may be < i0 in the first group)
         if (i >= i0 && i + 4 <= i1) {
             int4 tk, ps;
-            tk.x = token(i);
-            tk.y = token(i + 1);
-            tk.z = token(i + 2);
-            tk.w = token(i + 3);
+            int g = 0;
+            for (int kk = 1; kk < nseg; ++kk) g += (i >= cum[kk]) ? 1 : 0;
+            if (i + 4 <= cum[g + 1]) {  // the usual case: all four in one segment, one search
+                const int32_t* from = src[g] + i;
+                tk.x = __ldg(from);
+                tk.y = __ldg(from + 1);
+                tk.z = __ldg(from + 2);
+                tk.w = __ldg(from + 3);
+            } else {
+                tk.x = token(i);
+                tk.y = token(i + 1);
+                tk.z = token(i + 2);
+                tk.w = token(i + 3);
+            }
             ps = make_int4((int)i, (int)i + 1, (int)i + 2, (int)i + 3);
             __stcs(reinterpret_cast<int4*>(p.input_ids + o), tk);
             __stcs(reinterpret_cast<int4*>(p.position_ids + o), ps);
