@@ -288,7 +288,7 @@ def bench_gate_q24(torch, mosaic, pk):
             "achieved_gbs": byts / t / 1e9, "frac_of_measured_hbm": byts / t / 1e9 / pk["hbm_gbs"]}
 
 
-def bench_assemble(torch, mosaic, pk):
+def bench_assemble(torch, mosaic, pk, traffic=None):
     """SURVEY 8(f) N1 (a "next" row): mosaic_assemble_context over 2048 survivors of the C5 context
     recipe (U{8192..32768} tokens each, E = 8, prompt 256 + 8 traces at seeded cut points).
     Algorithmic bytes: 4 read + 8 written per token.  Parity: tests/test_gpu_assemble.py."""
@@ -330,7 +330,7 @@ def bench_assemble(torch, mosaic, pk):
     return {"workload": "SURVEY 8(f) N1: 2048 contexts of U{8192..32768} tokens, E=8", "tokens": T,
             "us_per_call": t * 1e6, "gtokens_per_s": T / t / 1e9,
             "roofline": {"bound": "hbm", "achieved": byts / t / 1e9, "peak": pk["hbm_gbs"],
-                         "unit": "GB/s", "frac": byts / t / 1e9 / pk["hbm_gbs"], "traffic": None,
+                         "unit": "GB/s", "frac": byts / t / 1e9 / pk["hbm_gbs"], "traffic": traffic,
                          "algorithmic_bytes": byts}}
 
 
@@ -442,7 +442,10 @@ def run_product(args):
         return
     gate_info = bench_gate_c5(torch, mosaic, wl, pk, steps=40, warmup=8)
     gate_info["q24"] = bench_gate_q24(torch, mosaic, pk)
-    assemble_info = bench_assemble(torch, mosaic, pk)
+    tj0 = ROOT / "profiles" / "traffic.json"
+    asm_traffic = (json.loads(tj0.read_text()).get("assemble_dram_bytes_per_launch")
+                   if tj0.exists() else None)
+    assemble_info = bench_assemble(torch, mosaic, pk, asm_traffic)
     f, t, threads, desc = oracle_sample(cfg, 0, args.cpu_rows)
     attn_tflops = flops / (attn_ms * 1e-3) / 1e12
     traffic = None
