@@ -153,6 +153,22 @@ def assemble_context(survivor_idx, cu_seqlens, prompt_tokens, prompt_off, trace_
     return dict(input_ids=ids, position_ids=pos, n_mismatch=n_mismatch)
 
 
+def rope(x, position_ids, theta: float):
+    """SURVEY.md 8(f) N1, second half: rotary position embedding of a packed [T, H, D] tensor
+    (binary64 values in, binary64 out; the caller rounds to bf16).  DESIGN.md reading N1-4: pairs
+    (i, i + D/2), w_i = theta^(-2i/D), a = position * w_i,
+    out[i] = x[i] cos a - x[i+D/2] sin a, out[i+D/2] = x[i+D/2] cos a + x[i] sin a."""
+    x = np.asarray(x, np.float64)
+    T, H, D = x.shape
+    pos = np.asarray(position_ids, np.float64).reshape(T)
+    half = D // 2
+    w = np.float64(theta) ** (-2.0 * np.arange(half, dtype=np.float64) / D)
+    a = pos[:, None] * w[None, :]                      # [T, D/2]
+    c, s = np.cos(a)[:, None, :], np.sin(a)[:, None, :]
+    lo, hi = x[..., :half], x[..., half:]
+    return np.concatenate([lo * c - hi * s, hi * c + lo * s], axis=-1)
+
+
 def _check_qkv(q, k, v, cu_seqlens):
     q = _c(q, np.uint16)
     k = _c(k, np.uint16)
