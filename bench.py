@@ -334,6 +334,35 @@ def bench_assemble(torch, mosaic, pk, traffic=None):
                          "algorithmic_bytes": byts}}
 
 
+def bench_rope(torch, mosaic, pk, T, Hq, Hkv, D):
+    """SURVEY 8(f) N1, second half: mosaic_rope_packed in place on a packed Q / K of the bench
+    config's shape (positions 0..L-1 of ~2 k-token sequences).  Algorithmic bytes: every element of
+    Q and K read and written once.  Parity: tests/test_gpu_rope.py."""
+    dev = "cuda"
+    g = torch.Generator(device=dev).manual_seed(41)
+    q = torch.randn((T, Hq, D), device=dev, generator=g).to(torch.bfloat16)
+    k = torch.randn((T, Hkv, D), device=dev, generator=g).to(torch.bfloat16)
+    pos = (torch.arange(T, device=dev, dtype=torch.int32) % 2090).contiguous()
+    for _ in range(2):
+        mosaic.rope_packed(q, k, pos, 1e6)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in range(5)]
+    torch.cuda.synchronize()
+    for e0, e1 in evs:   # 1.3 GB of Q + K: every call is L2-cold
+        e0.record()
+        mosaic.rope_packed(q, k, pos, 1e6)
+        e1.record()
+    torch.cuda.synchronize()
+    t = float(np.mean([e0.elapsed_time(e1) for e0, e1 in evs])) * 1e-3
+    byts = 4.0 * T * (Hq + Hkv) * D + 4.0 * T
+    return {"workload": "SURVEY 8(f) N1: RoPE in place on packed Q/K, T=%d, Hq/Hkv/D=%d/%d/%d" %
+                        (T, Hq, Hkv, D),
+            "us_per_call": t * 1e6, "gtokens_per_s": T / t / 1e9,
+            "roofline": {"bound": "hbm", "achieved": byts / t / 1e9, "peak": pk["hbm_gbs"],
+                         "unit": "GB/s", "frac": byts / t / 1e9 / pk["hbm_gbs"], "traffic": None,
+                         "algorithmic_bytes": byts}}
+
+
 def run_product(args):
     import torch
     import torch.distributed as dist
@@ -446,6 +475,7 @@ def run_product(args):
     asm_traffic = (json.loads(tj0.read_text()).get("assemble_dram_bytes_per_launch")
                    if tj0.exists() else None)
     assemble_info = bench_assemble(torch, mosaic, pk, asm_traffic)
+    rope_info = bench_rope(torch, mosaic, pk, T, cfg.Hq, cfg.Hkv, cfg.D)
     f, t, threads, desc = oracle_sample(cfg, 0, args.cpu_rows)
     attn_tflops = flops / (attn_ms * 1e-3) / 1e12
     traffic = None
@@ -470,6 +500,7 @@ def run_product(args):
                      "ms_per_launch": attn_ms, "peak_kind": "burst bf16_tflops"},
         "gate": gate_info,
         "assemble": assemble_info,
+        "rope": rope_info,
         "cpu_baseline": {"value": f / t / 1e12, "unit": UNIT, "cores": threads, "kind": "oracle",
                          "sample": desc},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d),

@@ -173,6 +173,22 @@ mosaic_status_t mosaic_assemble_context(const int32_t* survivor_idx, const int64
                                         int32_t* n_mismatch, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * mosaic_rope_packed -- SURVEY.md section 8(f) N1, second half: rotary position embedding applied
+ * IN PLACE to packed Q / K by the position_ids of mosaic_assemble_context.  The paper runs
+ * Qwen-family aggregators and does not describe the embedding; reading N1-4
+ * fixes those models' convention: pairs (i, i + D/2), w_i = theta^(-2i/D), a = position * w_i,
+ *     out[i] = x[i] cos a - x[i+D/2] sin a,   out[i+D/2] = x[i+D/2] cos a + x[i] sin a,
+ * angles and sin / cos in binary64, products in fp32, result rounded to nearest-even bf16.
+ *
+ *   q [dev] bf16 [total_tokens, Hq, D], k [dev] bf16 [total_tokens, Hkv, D]  in/out, 16-byte
+ *   aligned (either may be NULL when its head count is 0);  position_ids [dev] int32 [total_tokens];
+ *   D in {64, 128}; theta > 0 (e.g. 1e6).  Asynchronous on cuda_stream; nothing retained.
+ * ------------------------------------------------------------------------------------------- */
+mosaic_status_t mosaic_rope_packed(void* q, void* k, const int32_t* position_ids,
+                                   int64_t total_tokens, int32_t Hq, int32_t Hkv, int32_t D,
+                                   float theta, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * mosaic_stage_host -- the whole stage from HOST buffers (the end-to-end call): copies the gate
  * inputs to the device, runs mosaic_gate_compact, reads S / total_tokens / max_seqlen back,
  * copies the survivors' packed Q/K/V to the device, runs mosaic_agg_prefill_attn and copies every

@@ -32,6 +32,7 @@ SIGNATURES = {
                                                _i32, _f32, _vp, _vp, _vp, _sz, _vp]),
     "mosaic_assemble_context": (ctypes.c_int, [_vp, _vp, _i32, _i32, _vp, _vp, _vp, _vp, _i32, _vp,
                                                _vp, _vp, _vp]),
+    "mosaic_rope_packed": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _i32, _i32, _f32, _vp]),
     "mosaic_stage_host_arena_bytes": (_sz, [_i64, _i32, _i64, _i32, _i32, _i32]),
     "mosaic_stage_host": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _f32, _i32, _vp, _vp, _vp, _vp,
                                          _vp, _vp, _vp, _vp, _i32, _vp, _vp, _vp, _i64, _i32, _i32,
@@ -220,6 +221,17 @@ def assemble_context(survivor_idx, cu_seqlens, n_survivors, max_seqlen, total_to
         _stream(stream))
     _check("mosaic_assemble_context", st)
     return input_ids[:int(total_tokens)], position_ids[:int(total_tokens)], n_mismatch
+
+
+def rope_packed(q, k, position_ids, theta, *, stream=None):
+    """mosaic_rope_packed: rotates q bf16 [T,Hq,D] and k bf16 [T,Hkv,D] in place by position_ids."""
+    T, Hq, D = q.shape
+    Hkv = k.shape[1]
+    st = load().mosaic_rope_packed(_dptr(q, torch.bfloat16, "q"), _dptr(k, torch.bfloat16, "k"),
+                                   _dptr(position_ids, torch.int32, "position_ids"), int(T), Hq, Hkv,
+                                   D, float(theta), _stream(stream))
+    _check("mosaic_rope_packed", st)
+    return q, k
 
 
 def stage_host_arena_bytes(Q, E, T_cap, Hq, Hkv, D) -> int:
