@@ -334,7 +334,7 @@ def bench_assemble(torch, mosaic, pk, traffic=None):
                          "algorithmic_bytes": byts}}
 
 
-def bench_rope(torch, mosaic, pk, T, Hq, Hkv, D):
+def bench_rope(torch, mosaic, pk, T, Hq, Hkv, D, traffic=None):
     """SURVEY 8(f) N1, second half: mosaic_rope_packed in place on a packed Q / K of the bench
     config's shape (positions 0..L-1 of ~2 k-token sequences).  Algorithmic bytes: every element of
     Q and K read and written once.  Parity: tests/test_gpu_rope.py."""
@@ -359,7 +359,7 @@ def bench_rope(torch, mosaic, pk, T, Hq, Hkv, D):
                         (T, Hq, Hkv, D),
             "us_per_call": t * 1e6, "gtokens_per_s": T / t / 1e9,
             "roofline": {"bound": "hbm", "achieved": byts / t / 1e9, "peak": pk["hbm_gbs"],
-                         "unit": "GB/s", "frac": byts / t / 1e9 / pk["hbm_gbs"], "traffic": None,
+                         "unit": "GB/s", "frac": byts / t / 1e9 / pk["hbm_gbs"], "traffic": traffic,
                          "algorithmic_bytes": byts}}
 
 
@@ -475,7 +475,9 @@ def run_product(args):
     asm_traffic = (json.loads(tj0.read_text()).get("assemble_dram_bytes_per_launch")
                    if tj0.exists() else None)
     assemble_info = bench_assemble(torch, mosaic, pk, asm_traffic)
-    rope_info = bench_rope(torch, mosaic, pk, T, cfg.Hq, cfg.Hkv, cfg.D)
+    rope_traffic = (json.loads(tj0.read_text()).get("rope_dram_bytes_per_launch")
+                    if tj0.exists() else None)
+    rope_info = bench_rope(torch, mosaic, pk, T, cfg.Hq, cfg.Hkv, cfg.D, rope_traffic)
     f, t, threads, desc = oracle_sample(cfg, 0, args.cpu_rows)
     attn_tflops = flops / (attn_ms * 1e-3) / 1e12
     traffic = None
