@@ -18,7 +18,9 @@
 //     warps 0-3   : softmax of tile 0                   warps 4-7 : ... of tile 1
 //     warps 8-11  : epilogue of both tiles (O_t / l -> bf16 -> global, logsumexp), so that the
 //                   softmax groups go straight on to the next item
-//     warp 12     : TMA producer (Q tiles, K/V ring of kSlots 128-key tiles, 128-byte swizzle)
+//     warp 12     : TMA producer (Q tiles, K/V ring of kSlots 128-key tiles, 128-byte swizzle);
+//                   it also takes the CTA's next work unit from a global counter and publishes
+//                   it to the other roles through a small shared-memory ring
 //     warp 13, 14 : tcgen05.mma issuer of tile 0 / tile 1 (one elected thread each);
 //                   warp 14 also allocates / releases tensor memory
 //   Both softmax groups are busy all the time, so the FMA / ALU issue slots are as scarce as the
@@ -50,6 +52,7 @@ constexpr int BQ = 2 * BM;    // query rows per work item (two tiles)
 #endif
 constexpr int kSlots = MOSAIC_KV_SLOTS;  // K/V ring depth (tiles)
 constexpr int kThreadsAttn = 512;
+constexpr int kUnitSlots = 4;  // work units the producer may publish ahead of the other roles
 // Warp roles.  The softmax groups take the LOW warp ids (TMEM lane quarter = warp % 4) and the
 // single-thread roles the HIGH ones: the warp schedulers favour the highest warp id among the
 // eligible warps, and the MMA issuers are the threads everything else waits for.
@@ -68,8 +71,9 @@ constexpr int kPolyPairs = MOSAIC_POLY_PAIRS;  // of every 4 element pairs: exp2
 
 // ------------------------------------------------------------------------------- A5: schedule
 struct SchedHeader {
-    int n_items;  // number of (sequence, q block) entries
-    int pad[3];
+    int n_items;    // number of (sequence, q block) entries
+    int next_unit;  // work units handed out so far (attn_fwd's CTAs take them in cost order)
+    int pad[2];
 };
 
 struct Workspace {
@@ -174,7 +178,7 @@ __global__ void __launch_bounds__(1024) schedule_kernel(const int64_t* __restric
 struct AttnParams {
     const int64_t* cu_seqlens;
     const int4* items;
-    const SchedHeader* header;
+    SchedHeader* header;
     __nv_bfloat16* o;
     float* lse;
     int64_t T;
@@ -192,7 +196,8 @@ struct SmemLayout {
     static constexpr int kKV = 2 * kTileBytes;      // ring of kSlots tiles
     static constexpr int kBars = kKV + kSlots * kTileBytes;
     static constexpr int kStat = kBars + 512;       // (m, l) of every row of both tiles, for the epilogue
-    static constexpr int kTotal = kStat + 2 * BM * 8;
+    static constexpr int kUnits = kStat + 2 * BM * 8;  // ring of work-unit descriptors (32 bytes each)
+    static constexpr int kTotal = kUnits + kUnitSlots * 32;
     static constexpr int kDynamic = kTotal;         // the base is 1024-byte aligned (checked)
     static_assert(kDynamic <= 227 * 1024, "shared memory of one CTA");
 };
@@ -209,7 +214,9 @@ enum Bar : uint32_t {
     kBarODone = kBarSFull + 10,             // [2]  last PV_t of the item complete   (commit)
     kBarStat = kBarSFull + 12,              // [2]  (m, l) of the tile's rows are in shared memory (4 warps)
     kBarOFree = kBarSFull + 14,             // [2]  the epilogue has read O_t        (4 warps)
-    kNumBars = kBarSFull + 16
+    kBarUnitFull = kBarSFull + 16,          // [kUnitSlots] the producer has published a work unit
+    kBarUnitEmpty = kBarSFull + 16 + kUnitSlots,  // [kUnitSlots] every other role has read it (14 warps)
+    kNumBars = kBarSFull + 16 + 2 * kUnitSlots
 };
 static_assert(kNumBars * 8 + 8 <= 512, "barrier region");
 
@@ -224,42 +231,29 @@ struct Work {
     __device__ __forceinline__ int n(int t) const { return t ? n1 : n0; }
 };
 
-// The work units of one CTA: w = blockIdx.x, + gridDim.x, ...; unit w is q head w % Hq of entry
-// w / Hq of the work list.  (entry, head) are stepped, not divided out, and the descriptor of a
-// unit is loaded one unit ahead and decoded only when the unit starts, so the load (an L2 round
-// trip) hides behind the unit before it.
-struct WorkCursor {
-    int item, h, d_item, d_h;
-    int4 it;
-    __device__ __forceinline__ WorkCursor(const AttnParams& p, int n_work) {
-        item = (int)blockIdx.x / p.Hq;
-        h = (int)blockIdx.x - item * p.Hq;
-        d_item = (int)gridDim.x / p.Hq;
-        d_h = (int)gridDim.x - d_item * p.Hq;
-        it = make_int4(0, 0, 0, 0);
-        if ((int)blockIdx.x < n_work) it = __ldg(p.items + item);
-    }
-    // the current unit; `more`: there is a next one (its descriptor is requested now)
-    __device__ __forceinline__ Work take(const AttnParams& p, bool more) {
-        Work k;
-        k.h = h;
-        k.g = __float2int_rd(((float)h + 0.5f) * p.inv_group);  // h / (Hq / Hkv)
-        k.t0 = it.x;
-        k.L = it.y;
-        k.row0 = it.z * BQ;
-        k.n0 = 2 * it.z + 1;
-        k.n1 = (k.row0 + BM < k.L) ? 2 * it.z + 2 : 0;
-        k.n_kv = max(k.n0, k.n1);
-        item += d_item;
-        h += d_h;
-        if (h >= p.Hq) {
-            h -= p.Hq;
-            ++item;
-        }
-        if (more) it = __ldg(p.items + item);
-        return k;
-    }
+// Work units (unit w = q head w % Hq of entry w / Hq of the cost-sorted work list) are handed out
+// dynamically: the producer warp of a CTA takes the next unit from a global counter, loads its
+// descriptor and publishes both in a small shared-memory ring that every other warp role reads,
+// so all roles of a CTA walk the same sequence, and a CTA that runs faster (the per-CTA finish
+// times of a static assignment spread over 5 % of the kernel) simply takes more units.
+constexpr int kUnitConsumers = 14;  // 8 softmax + 4 epilogue + 2 issuer warps
+struct UnitEntry {  // 32 bytes in shared memory
+    int4 it;        // (first token, length, q block, sequence) of the entry
+    int h;          // q head; < 0: no more work
+    int pad[3];
 };
+__device__ __forceinline__ Work make_work(const AttnParams& p, const int4 it, int h) {
+    Work k;
+    k.h = h;
+    k.g = __float2int_rd(((float)h + 0.5f) * p.inv_group);  // h / (Hq / Hkv)
+    k.t0 = it.x;
+    k.L = it.y;
+    k.row0 = it.z * BQ;
+    k.n0 = 2 * it.z + 1;
+    k.n1 = (k.row0 + BM < k.L) ? 2 * it.z + 2 : 0;
+    k.n_kv = max(k.n0, k.n1);
+    return k;
+}
 
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;
@@ -333,6 +327,10 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             for (int s = 0; s < kSlots; ++s) ptx::mbar_init(bar_kv_empty(t, s), 1);
         }
         for (int s = 0; s < kSlots; ++s) ptx::mbar_init(bar(kBarKvFull, s), 1);
+        for (int s = 0; s < kUnitSlots; ++s) {
+            ptx::mbar_init(bar(kBarUnitFull, s), 1);
+            ptx::mbar_init(bar(kBarUnitEmpty, s), kUnitConsumers);
+        }
         asm volatile("st.shared.u32 [%0], %1;" ::"r"(mma_lock), "r"(0u) : "memory");
         ptx::fence_barrier_init();
     }
@@ -344,6 +342,26 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
     __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+
+    // The next work unit of this CTA, as published by the producer warp (whole warp calls; false
+    // when there is no more work).  n counts the units this warp has read.
+    volatile UnitEntry* unit_ring = reinterpret_cast<volatile UnitEntry*>(smem + SL::kUnits);
+    auto next_unit = [&](uint32_t& n, Work& k) -> bool {
+        const uint32_t slot = n % kUnitSlots, ph = (n / kUnitSlots) & 1u;
+        ++n;
+        ptx::mbar_wait(bar(kBarUnitFull, (int)slot), ph);
+        int4 it;
+        it.x = unit_ring[slot].it.x;
+        it.y = unit_ring[slot].it.y;
+        it.z = unit_ring[slot].it.z;
+        it.w = unit_ring[slot].it.w;
+        const int h = unit_ring[slot].h;
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(bar(kBarUnitEmpty, (int)slot));
+        if (h < 0) return false;
+        k = make_work(p, it, h);
+        return true;
+    };
 
     // Position q of the K/V ring sequence (K_0, V_0, K_1, V_1, ... of one item after the other)
     // lives in slot q % kSlots; its full / empty barriers are in phase (q / kSlots) & 1.
@@ -358,9 +376,8 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
             const float2* stat = reinterpret_cast<const float2*>(smem + SL::kStat);
             uint32_t ph[2] = {0, 0};
-            WorkCursor cursor(p, n_work);
-            for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-                const Work k = cursor.take(p, w + (int)gridDim.x < n_work);
+            uint32_t n_units = 0;
+            for (Work k; next_unit(n_units, k);) {
 #pragma unroll 1
                 for (int t = 0; t < 2; ++t) {
                     if (k.n(t) == 0) continue;
@@ -413,9 +430,42 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         } else if (warp == kWarpProducer) {
             // ================================ TMA producer ================================
             uint32_t pos = 0, ph_q[2] = {0, 0};
-            WorkCursor cursor(p, n_work);
-            for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-                const Work k = cursor.take(p, w + (int)gridDim.x < n_work);
+            // Units are fetched one ahead (counter and descriptor: two L2 round trips that hide
+            // behind the unit in progress) and published when their turn comes.
+            uint32_t n_pub = 0;
+            int4 f_it = make_int4(0, 0, 0, 0);
+            int f_h = -1;
+            auto fetch = [&]() {
+                int w = 0;
+                if (lane == 0) w = atomicAdd(&p.header->next_unit, 1);
+                w = __shfl_sync(0xffffffffu, w, 0);
+                f_h = -1;
+                if (w < n_work) {
+                    const int item = w / p.Hq;
+                    f_h = w - item * p.Hq;
+                    f_it = __ldg(p.items + item);
+                }
+            };
+            auto publish = [&]() {  // the fetched unit (or the end marker) to every other role
+                const uint32_t slot = n_pub % kUnitSlots, ph = (n_pub / kUnitSlots) & 1u;
+                ++n_pub;
+                ptx::mbar_wait(bar(kBarUnitEmpty, (int)slot), ph ^ 1);
+                if (lane == 0) {
+                    unit_ring[slot].it.x = f_it.x;
+                    unit_ring[slot].it.y = f_it.y;
+                    unit_ring[slot].it.z = f_it.z;
+                    unit_ring[slot].it.w = f_it.w;
+                    unit_ring[slot].h = f_h;
+                    ptx::mbar_arrive(bar(kBarUnitFull, (int)slot));
+                }
+                __syncwarp();
+            };
+            fetch();
+            for (;;) {
+                publish();
+                if (f_h < 0) break;
+                const Work k = make_work(p, f_it, f_h);
+                fetch();  // the unit after this one
                 auto load_q = [&](int t) {
                     ptx::mbar_wait(bar(kBarQEmpty, t), ph_q[t] ^ 1);
                     ph_q[t] ^= 1;
@@ -512,9 +562,8 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             // so S(u+2) overwrites P(u) right behind PV(u) in the (in-order) tensor pipe and is
             // ready, as a rule, before the softmax group has finished step u + 1.
             uint32_t pos = 0, ph_q = 0, ph_p = 0, ph_f = 0;
-            WorkCursor cursor(p, n_work);
-            for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-                const Work k = cursor.take(p, w + (int)gridDim.x < n_work);
+            uint32_t n_units = 0;
+            for (Work k; next_unit(n_units, k);) {
                 const int n_t = k.n(t);
                 const uint32_t base = pos;
                 if (n_t > 0) {
@@ -709,9 +758,8 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         using M1 = std::integral_constant<int, 1>;
         using M2 = std::integral_constant<int, 2>;
 
-        WorkCursor cursor(p, n_work);
-        for (int w = blockIdx.x; w < n_work; w += gridDim.x) {
-            const Work k = cursor.take(p, w + (int)gridDim.x < n_work);
+        uint32_t n_units = 0;
+        for (Work k; next_unit(n_units, k);) {
             const int n_t = k.n(t);
             if (n_t == 0) continue;  // this tile has no rows in this block
             m_used = 0.f;
