@@ -115,6 +115,43 @@ def compact(bypass, ctx_len):
                 total_tokens=int(tot[0]), max_seqlen=int(mx[0]))
 
 
+def attn_kv_full(q, k, v, cu_seqlens_q, cu_seqlens_k, softmax_scale):
+    """SURVEY.md 8(f) N2 (prefix-cached / chunked prefill): the q rows of a sequence are the LAST
+    Lq of its Lk positions, so row i sees keys j <= i + (Lk - Lq) ("bottom-right" causal alignment,
+    DESIGN.md reading N2-1; Lk = Lq is the plain prefill of north_star).  The definition written
+    out per (sequence, q head) with numpy in binary64: S = scale Q K^T, mask, row softmax, O = P V,
+    LSE = ln sum_j exp(S_ij).  q uint16 [Tq,Hq,D], k/v uint16 [Tk,Hkv,D] (bf16 bits).
+    Returns (O float64 [Tq,Hq,D], LSE float64 [Hq,Tq])."""
+    def f64(bits):
+        return (_c(bits, np.uint16).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+    Q, K, V = f64(q), f64(k), f64(v)
+    cq, ck = _c(cu_seqlens_q, np.int64), _c(cu_seqlens_k, np.int64)
+    Tq, Hq, D = Q.shape
+    Hkv = K.shape[1]
+    assert cq.shape == ck.shape and Hq % Hkv == 0
+    O = np.zeros((Tq, Hq, D), np.float64)
+    lse = np.zeros((Hq, Tq), np.float64)
+    scale = float(np.float32(softmax_scale))
+    for s_ in range(cq.shape[0] - 1):
+        a, b = int(cq[s_]), int(cq[s_ + 1])
+        c, d = int(ck[s_]), int(ck[s_ + 1])
+        Lq, Lk = b - a, d - c
+        if Lq == 0:
+            continue
+        assert Lk >= Lq
+        visible = np.arange(Lk)[None, :] <= (np.arange(Lq)[:, None] + (Lk - Lq))
+        for h in range(Hq):
+            g = h // (Hq // Hkv)
+            S = scale * (Q[a:b, h] @ K[c:d, g].T)
+            S = np.where(visible, S, -np.inf)
+            M = S.max(axis=1, keepdims=True)
+            P = np.exp(S - M)
+            Z = P.sum(axis=1, keepdims=True)
+            O[a:b, h] = (P / Z) @ V[c:d, g]
+            lse[h, a:b] = (M + np.log(Z))[:, 0]
+    return O, lse
+
+
 def assemble_context(survivor_idx, cu_seqlens, prompt_tokens, prompt_off, trace_tokens, trace_off,
                      E: int):
     """the survivors' aggregator contexts as one packed token batch.  The
