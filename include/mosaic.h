@@ -146,6 +146,31 @@ mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k, const void
                                         void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * mosaic_agg_prefill_attn_kv -- SURVEY.md section 8(f) N2 (a "next" row): the same attention with
+ * the q rows and the keys of a sequence packed separately, for prefix-cached prompts and chunked
+ * prefill of the aggregator's long contexts (32 k-class windows): sequence s has Lq q rows
+ * (cu_seqlens_q) and Lk >= Lq keys (cu_seqlens_k), the q rows being the LAST Lq positions, so
+ * row i sees keys j <= i + (Lk - Lq) ("bottom-right" causal alignment, reading N2-1).
+ * Lk = Lq for every sequence is mosaic_agg_prefill_attn.  Together with the exported LSE this is
+ * what split-KV / chunked prefill merges are built from.
+ *
+ *   q [dev] bf16 [total_q_tokens, Hq, D]; k, v [dev] bf16 [total_k_tokens, Hkv, D];
+ *   cu_seqlens_q, cu_seqlens_k [dev] int64 [n_seqs + 1]; max_seqlen_q >= every Lq;
+ *   o [dev] bf16 [total_q_tokens, Hq, D]; lse [dev] fp32 [Hq, total_q_tokens];
+ *   workspace >= mosaic_agg_prefill_attn_workspace_bytes(n_seqs, total_q_tokens, ...).
+ * Everything else (alignment, D, errors, asynchrony) as mosaic_agg_prefill_attn.  Lk < Lq is not
+ * checked and not supported.
+ * ------------------------------------------------------------------------------------------- */
+mosaic_status_t mosaic_agg_prefill_attn_kv(const void* q, const void* k, const void* v,
+                                           const int64_t* cu_seqlens_q,
+                                           const int64_t* cu_seqlens_k, int32_t n_seqs,
+                                           int64_t total_q_tokens, int64_t total_k_tokens,
+                                           int32_t max_seqlen_q, int32_t Hq, int32_t Hkv, int32_t D,
+                                           float softmax_scale, void* o, float* lse,
+                                           void* workspace, size_t workspace_bytes,
+                                           void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * mosaic_assemble_context -- SURVEY.md section 8(f) N1 (a "next" row, between G5 and A1): the
  * survivors' aggregator contexts as one packed token batch.  The aggregator "process[es] the
  * combined output or reasoning traces of its experts" (Alg. 1

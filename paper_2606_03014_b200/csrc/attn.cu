@@ -81,7 +81,8 @@ struct Workspace {
     int* cnt;     // [levels]  sequences with exactly c+1 q blocks -> sequences with more than c
     int* start;   // [levels]  first entry of level c (levels in descending order)
     int* cursor;  // [levels]
-    int4* items;  // [capacity] (first token of the sequence, its length, q block, sequence)
+    int4* items;  // [capacity] (first q token of the sequence, its q length, q block, first k token)
+    int* items_lk;  // [capacity] its k length
     size_t zero_bytes;  // prefix that must be zeroed before schedule_kernel
     size_t total_bytes;
 };
@@ -104,6 +105,8 @@ inline Workspace carve(void* base, int32_t n_seqs, int64_t total_tokens) {
     off = (off + 15) & ~size_t(15);
     w.items = reinterpret_cast<int4*>(p + off);
     off += cap * sizeof(int4);
+    w.items_lk = reinterpret_cast<int*>(p + off);
+    off += cap * sizeof(int);
     w.total_bytes = (off + 255) & ~size_t(255);
     return w;
 }
@@ -132,9 +135,10 @@ __device__ __forceinline__ int block_suffix_exclusive(int v, int* warp_tot /* [3
 }
 
 __global__ void __launch_bounds__(1024) schedule_kernel(const int64_t* __restrict__ cu_seqlens,
+                                                        const int64_t* __restrict__ cu_seqlens_k,
                                                         int n_seqs, int levels, SchedHeader* header,
                                                         int* cnt, int* start, int* cursor,
-                                                        int4* items) {
+                                                        int4* items, int* items_lk) {
     __shared__ int warp_tot[32];
     const int tid = threadIdx.x;
     for (int s = tid; s < n_seqs; s += blockDim.x) {
@@ -167,9 +171,12 @@ __global__ void __launch_bounds__(1024) schedule_kernel(const int64_t* __restric
         const int64_t L = cu_seqlens[s + 1] - cu_seqlens[s];
         const int nb = min((int)((L + BQ - 1) / BQ), levels);
         const int t0 = (int)cu_seqlens[s];  // total_tokens < 2^31
+        const int tk0 = (int)cu_seqlens_k[s];
+        const int Lk = (int)(cu_seqlens_k[s + 1] - cu_seqlens_k[s]);
         for (int c = 0; c < nb; ++c) {
             const int at = start[c] + atomicAdd(&cursor[c], 1);
-            items[at] = make_int4(t0, (int)L, c, s);  // everything a CTA needs, in one load
+            items[at] = make_int4(t0, (int)L, c, tk0);  // everything a CTA needs
+            items_lk[at] = Lk;
         }
     }
 }
@@ -178,6 +185,7 @@ __global__ void __launch_bounds__(1024) schedule_kernel(const int64_t* __restric
 struct AttnParams {
     const int64_t* cu_seqlens;
     const int4* items;
+    const int* items_lk;
     SchedHeader* header;
     __nv_bfloat16* o;
     float* lse;
@@ -223,12 +231,15 @@ static_assert(kNumBars * 8 + 8 <= 512, "barrier region");
 // One (work item, q head) pair as every warp role sees it.
 struct Work {
     int h, g;        // q head, kv head
-    int64_t t0;      // first token of the sequence
-    int L;           // sequence length
+    int64_t t0;      // first q token of the sequence
+    int64_t tk0;     // first k token of the sequence
+    int L;           // q rows of the sequence
+    int off;         // k length - q length: row i sees keys j <= i + off (0 for plain prefill)
     int row0;        // first row of the block inside the sequence
     int n0, n1;      // KV tiles of tile 0 / tile 1 (0 = tile has no rows)
     int n_kv;        // max of the two
     __device__ __forceinline__ int n(int t) const { return t ? n1 : n0; }
+    __device__ __forceinline__ int tile_of(int t) const { return t; }
 };
 
 // Work units (unit w = q head w % Hq of entry w / Hq of the cost-sorted work list) are handed out
@@ -238,19 +249,24 @@ struct Work {
 // times of a static assignment spread over 5 % of the kernel) simply takes more units.
 constexpr int kUnitConsumers = 14;  // 8 softmax + 4 epilogue + 2 issuer warps
 struct UnitEntry {  // 32 bytes in shared memory
-    int4 it;        // (first token, length, q block, sequence) of the entry
+    int4 it;        // (first q token, q length, q block, first k token) of the entry
     int h;          // q head; < 0: no more work
-    int pad[3];
+    int lk;         // k length of the entry
+    int pad[2];
 };
-__device__ __forceinline__ Work make_work(const AttnParams& p, const int4 it, int h) {
+__device__ __forceinline__ Work make_work(const AttnParams& p, const int4 it, int h, int lk) {
     Work k;
     k.h = h;
     k.g = __float2int_rd(((float)h + 0.5f) * p.inv_group);  // h / (Hq / Hkv)
     k.t0 = it.x;
+    k.tk0 = it.w;
     k.L = it.y;
+    k.off = lk - it.y;
     k.row0 = it.z * BQ;
-    k.n0 = 2 * it.z + 1;
-    k.n1 = (k.row0 + BM < k.L) ? 2 * it.z + 2 : 0;
+    // KV tiles of a q tile: up to the last key its last row sees (2c+1 and 2c+2 when off = 0)
+    const int last0 = min(k.row0 + BM, k.L) + k.off, last1 = min(k.row0 + BQ, k.L) + k.off;
+    k.n0 = (last0 + BN - 1) / BN;
+    k.n1 = (k.row0 + BM < k.L) ? (last1 + BN - 1) / BN : 0;
     k.n_kv = max(k.n0, k.n1);
     return k;
 }
@@ -356,10 +372,11 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         it.z = unit_ring[slot].it.z;
         it.w = unit_ring[slot].it.w;
         const int h = unit_ring[slot].h;
+        const int lk = unit_ring[slot].lk;
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(bar(kBarUnitEmpty, (int)slot));
         if (h < 0) return false;
-        k = make_work(p, it, h);
+        k = make_work(p, it, h, lk);
         return true;
     };
 
@@ -434,7 +451,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             // behind the unit in progress) and published when their turn comes.
             uint32_t n_pub = 0;
             int4 f_it = make_int4(0, 0, 0, 0);
-            int f_h = -1;
+            int f_h = -1, f_lk = 0;
             auto fetch = [&]() {
                 int w = 0;
                 if (lane == 0) w = atomicAdd(&p.header->next_unit, 1);
@@ -444,6 +461,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                     const int item = w / p.Hq;
                     f_h = w - item * p.Hq;
                     f_it = __ldg(p.items + item);
+                    f_lk = __ldg(p.items_lk + item);
                 }
             };
             auto publish = [&]() {  // the fetched unit (or the end marker) to every other role
@@ -456,6 +474,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                     unit_ring[slot].it.z = f_it.z;
                     unit_ring[slot].it.w = f_it.w;
                     unit_ring[slot].h = f_h;
+                    unit_ring[slot].lk = f_lk;
                     ptx::mbar_arrive(bar(kBarUnitFull, (int)slot));
                 }
                 __syncwarp();
@@ -464,7 +483,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             for (;;) {
                 publish();
                 if (f_h < 0) break;
-                const Work k = make_work(p, f_it, f_h);
+                const Work k = make_work(p, f_it, f_h, f_lk);
                 fetch();  // the unit after this one
                 auto load_q = [&](int t) {
                     ptx::mbar_wait(bar(kBarQEmpty, t), ph_q[t] ^ 1);
@@ -490,7 +509,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                         for (int c = 0; c < D / 64; ++c)
                             ptx::tma_load_3d(sKV + slot * SL::kTileBytes + c * SL::kBlockBytes, tm,
                                              bar(kBarKvFull, slot), c * 64, k.g,
-                                             (int)(k.t0 + j * BN));
+                                             (int)(k.tk0 + j * BN));
                     }
                     __syncwarp();
                 };
@@ -646,9 +665,11 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         const float sc = p.scale_log2;
         uint32_t ph_s = 0, ph_f = 0;
         float m_used = 0.f, l_run = 0.f;
+        int thr = 0;  // of the masked step in progress
 
         // One step: 64 scores of this row (buffer b) -> running max -> P (bf16, in place) -> row sum.
-        //   kMask 0: no key masked   1: keys 64 b + c > row masked   2: every key masked (warp-uniform)
+        //   kMask 0: no key masked   1: keys c > thr masked (thr = last key this row sees, relative
+        //   to the step's first key)   2: every key masked (warp-uniform)
         // (Every call site is a copy of ~500 unrolled instructions and the instruction cache is
         //  small: the steady state gets one copy per buffer with b a constant, the two steps of
         //  the diagonal tile share one masked copy with b a run-time value.)
@@ -674,7 +695,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                 if constexpr (kMask == 1) {
 #pragma unroll
                     for (int c = 0; c < BS; ++c)
-                        if (c > row - b * BS) s[c] = -INFINITY;
+                        if (c > thr) s[c] = -INFINITY;
                 }
                 float mx0 = s[0], mx1 = s[1], mx2 = s[2], mx3 = s[3];
 #pragma unroll
@@ -764,22 +785,29 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             if (n_t == 0) continue;  // this tile has no rows in this block
             m_used = 0.f;
             l_run = 0.f;
-            // The last two steps are the diagonal tile: key 64 b + c is masked for query row r when
-            // 64 b + c > r.  Per warp (32 rows) a 64-key half is untouched (rows 64-127, b = 0),
-            // partly masked (rows 0-63, b = 0; rows 64-127, b = 1) or masked altogether (rows 0-63,
-            // b = 1).
-            for (int j = 0; j + 1 < n_t; ++j) {
-                step(M0{}, 0, j == 0);
+            // Row r of the sequence sees keys j <= r + off.  Steps whose 64 keys every row of the tile
+            // sees run unmasked, in pairs (one copy per buffer); from the first step that some row of
+            // the tile does not see in full, a warp's 32 rows x 64 keys are either masked altogether
+            // or go through the masked copy with thr = r + off - 64 u (which masks nothing when
+            // thr >= 63).  With off = 0 these are the two steps of the diagonal tile: untouched for
+            // rows 64-127 at b = 0, masked altogether for rows 0-63 at b = 1, partly masked otherwise.
+            const int tile_row0 = k.row0 + k.tile_of(t) * BM;  // first row of the tile in the sequence
+            const int u_masked = ((tile_row0 + k.off + 1) >> 6) & ~1;
+            const int U = 2 * n_t;
+            for (int u = 0; u < u_masked; u += 2) {
+                step(M0{}, 0, u == 0);
                 step(M0{}, 1, false);
                 ph_s ^= 1;
             }
-            for (int b = 0; b < 2; ++b) {
-                if (b == 1 && wq < 2)
+            for (int u = u_masked; u < U; ++u) {
+                const int b = u & 1;
+                thr = tile_row0 + row + k.off - u * BS;
+                if (tile_row0 + wq * 32 + 31 + k.off - u * BS < 0)
                     step(M2{}, b, false);
                 else
-                    step(M1{}, b, b == 0 && n_t == 1);  // (masks nothing for rows 64-127, b = 0)
+                    step(M1{}, b, u == 0);
+                ph_s ^= (uint32_t)b;
             }
-            ph_s ^= 1;
             // ---- hand the row's (m, l) to the epilogue warps and go on to the next item -----------
             // (first make sure the epilogue has read the previous item's pair -- it releases O_t
             //  after that; an item of a single KV tile gets here without PV_t(0) having waited)
@@ -860,19 +888,21 @@ extern "C" size_t mosaic_agg_prefill_attn_workspace_bytes(int32_t n_seqs, int64_
     return carve(nullptr, n_seqs, total_tokens).total_bytes;
 }
 
-extern "C" mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k, const void* v,
-                                                   const int64_t* cu_seqlens, int32_t n_seqs,
-                                                   int64_t total_tokens, int32_t max_seqlen,
-                                                   int32_t Hq, int32_t Hkv, int32_t D,
-                                                   float softmax_scale, void* o, float* lse,
-                                                   void* workspace, size_t workspace_bytes,
-                                                   void* cuda_stream) {
-    if (n_seqs < 0 || total_tokens < 0 || total_tokens >= (1ll << 31) || max_seqlen < 0 ||
-        Hq < 1 || Hkv < 1 || Hq % Hkv != 0 || !isfinite(softmax_scale))
+namespace {
+// q rows and keys may be packed separately (cu_seqlens / total_tokens for q, O and LSE;
+// cu_seqlens_k / total_k_tokens for K and V); the plain prefill passes the same for both.
+mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int64_t* cu_seqlens,
+                          const int64_t* cu_seqlens_k, int32_t n_seqs, int64_t total_tokens,
+                          int64_t total_k_tokens, int32_t max_seqlen, int32_t Hq, int32_t Hkv,
+                          int32_t D, float softmax_scale, void* o, float* lse, void* workspace,
+                          size_t workspace_bytes, void* cuda_stream) {
+    if (n_seqs < 0 || total_tokens < 0 || total_tokens >= (1ll << 31) || total_k_tokens < 0 ||
+        total_k_tokens >= (1ll << 31) || max_seqlen < 0 || Hq < 1 || Hkv < 1 || Hq % Hkv != 0 ||
+        !isfinite(softmax_scale))
         return MOSAIC_ERR_INVALID_ARG;
     if (D != 64 && D != 128) return MOSAIC_ERR_UNSUPPORTED;
     if (n_seqs == 0 || total_tokens == 0) return MOSAIC_OK;
-    if (!q || !k || !v || !o || !lse || !cu_seqlens || !workspace || !aligned16(q) ||
+    if (!q || !k || !v || !o || !lse || !cu_seqlens || !cu_seqlens_k || !workspace || !aligned16(q) ||
         !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(workspace))
         return MOSAIC_ERR_INVALID_ARG;
     Workspace w = carve(workspace, n_seqs, total_tokens);
@@ -881,20 +911,21 @@ extern "C" mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k,
 
     CUtensorMap tq, tk, tv;
     if (!make_tensor_map(&tq, q, total_tokens, Hq, D, BM) ||
-        !make_tensor_map(&tk, k, total_tokens, Hkv, D, BN) ||
-        !make_tensor_map(&tv, v, total_tokens, Hkv, D, BN))
+        !make_tensor_map(&tk, k, total_k_tokens, Hkv, D, BN) ||
+        !make_tensor_map(&tv, v, total_k_tokens, Hkv, D, BN))
         return MOSAIC_ERR_CUDA;
 
     const int levels = (int)(total_tokens / BQ) + 2;
     MOSAIC_CUDA_TRY(cudaMemsetAsync(workspace, 0, w.zero_bytes, s));
-    schedule_kernel<<<1, 1024, 0, s>>>(cu_seqlens, n_seqs, levels, w.header, w.cnt, w.start,
-                                       w.cursor, w.items);
+    schedule_kernel<<<1, 1024, 0, s>>>(cu_seqlens, cu_seqlens_k, n_seqs, levels, w.header, w.cnt,
+                                       w.start, w.cursor, w.items, w.items_lk);
     count_launch();
     MOSAIC_CUDA_TRY(cudaGetLastError());
 
     AttnParams p{};
     p.cu_seqlens = cu_seqlens;
     p.items = w.items;
+    p.items_lk = w.items_lk;
     p.header = w.header;
     p.o = static_cast<__nv_bfloat16*>(o);
     p.lse = lse;
@@ -910,4 +941,26 @@ extern "C" mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k,
     const int grid = (int)(max_work < num_sms() ? max_work : num_sms());
     return D == 64 ? launch_attn<64>(tq, tk, tv, p, negate_q, grid, s)
                    : launch_attn<128>(tq, tk, tv, p, negate_q, grid, s);
+}
+}  // namespace
+
+extern "C" mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k, const void* v,
+                                                   const int64_t* cu_seqlens, int32_t n_seqs,
+                                                   int64_t total_tokens, int32_t max_seqlen,
+                                                   int32_t Hq, int32_t Hkv, int32_t D,
+                                                   float softmax_scale, void* o, float* lse,
+                                                   void* workspace, size_t workspace_bytes,
+                                                   void* cuda_stream) {
+    return attn_impl(q, k, v, cu_seqlens, cu_seqlens, n_seqs, total_tokens, total_tokens, max_seqlen,
+                     Hq, Hkv, D, softmax_scale, o, lse, workspace, workspace_bytes, cuda_stream);
+}
+
+extern "C" mosaic_status_t mosaic_agg_prefill_attn_kv(
+    const void* q, const void* k, const void* v, const int64_t* cu_seqlens_q,
+    const int64_t* cu_seqlens_k, int32_t n_seqs, int64_t total_q_tokens, int64_t total_k_tokens,
+    int32_t max_seqlen_q, int32_t Hq, int32_t Hkv, int32_t D, float softmax_scale, void* o,
+    float* lse, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    return attn_impl(q, k, v, cu_seqlens_q, cu_seqlens_k, n_seqs, total_q_tokens, total_k_tokens,
+                     max_seqlen_q, Hq, Hkv, D, softmax_scale, o, lse, workspace, workspace_bytes,
+                     cuda_stream);
 }

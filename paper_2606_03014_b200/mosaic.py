@@ -30,6 +30,8 @@ SIGNATURES = {
     "mosaic_agg_prefill_attn_workspace_bytes": (_sz, [_i32, _i64, _i32, _i32, _i32]),
     "mosaic_agg_prefill_attn": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i64, _i32, _i32, _i32,
                                                _i32, _f32, _vp, _vp, _vp, _sz, _vp]),
+    "mosaic_agg_prefill_attn_kv": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _i32, _i64, _i64, _i32,
+                                                  _i32, _i32, _i32, _f32, _vp, _vp, _vp, _sz, _vp]),
     "mosaic_assemble_context": (ctypes.c_int, [_vp, _vp, _i32, _i32, _vp, _vp, _vp, _vp, _i32, _vp,
                                                _vp, _vp, _vp]),
     "mosaic_rope_packed": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _i32, _i32, _f32, _vp]),
@@ -197,6 +199,32 @@ def agg_prefill_attn(q, k, v, cu_seqlens, n_seqs, max_seqlen, softmax_scale, *, 
         D, float(softmax_scale), _dptr(o, torch.bfloat16, "o"), _dptr(lse, torch.float32, "lse"),
         _dptr(workspace), workspace.numel(), _stream(stream))
     _check("mosaic_agg_prefill_attn", st)
+    return o, lse
+
+
+def agg_prefill_attn_kv(q, k, v, cu_seqlens_q, cu_seqlens_k, n_seqs, max_seqlen_q, softmax_scale, *,
+                        o=None, lse=None, workspace=None, stream=None):
+    """mosaic_agg_prefill_attn_kv: q bf16 [Tq,Hq,D], k/v bf16 [Tk,Hkv,D],
+    row i of a sequence sees keys j <= i + (Lk - Lq).  Returns (o bf16 [Tq,Hq,D], lse fp32 [Hq,Tq])."""
+    Tq, Hq, D = q.shape
+    Tk, Hkv = k.shape[0], k.shape[1]
+    if k.shape != (Tk, Hkv, D) or v.shape != k.shape:
+        raise ValueError("k/v shape")
+    dev = q.device
+    if o is None:
+        o = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty((Hq, Tq), dtype=torch.float32, device=dev)
+    if workspace is None:
+        workspace = torch.empty(max(attn_workspace_bytes(n_seqs, Tq, Hq, Hkv, D), 16),
+                                dtype=torch.uint8, device=dev)
+    st = load().mosaic_agg_prefill_attn_kv(
+        _dptr(q, torch.bfloat16, "q"), _dptr(k, torch.bfloat16, "k"), _dptr(v, torch.bfloat16, "v"),
+        _dptr(cu_seqlens_q, torch.int64, "cu_seqlens_q"), _dptr(cu_seqlens_k, torch.int64, "cu_seqlens_k"),
+        int(n_seqs), int(Tq), int(Tk), int(max_seqlen_q), Hq, Hkv, D, float(softmax_scale),
+        _dptr(o, torch.bfloat16, "o"), _dptr(lse, torch.float32, "lse"), _dptr(workspace),
+        workspace.numel(), _stream(stream))
+    _check("mosaic_agg_prefill_attn_kv", st)
     return o, lse
 
 
