@@ -363,6 +363,42 @@ def bench_rope(torch, mosaic, pk, T, Hq, Hkv, D, traffic=None):
                          "algorithmic_bytes": byts}}
 
 
+def bench_attn_kv(torch, mosaic, pk):
+    """the last 8192 q rows of two 32768-token contexts against all their keys
+    (the last chunk of a chunked prefill), Hq/Hkv/D = 32/8/128.  Algorithmic flops: 4 Hq D per
+    visible (row, key) pair.  Parity: tests/test_gpu_attn_kv.py."""
+    Lq, Lk, n, Hq, Hkv, D = 8192, 32768, 2, 32, 8, 128
+    dev = "cuda"
+    g = torch.Generator(device=dev).manual_seed(51)
+    q = torch.randn((n * Lq, Hq, D), device=dev, generator=g).to(torch.bfloat16)
+    k = torch.randn((n * Lk, Hkv, D), device=dev, generator=g).to(torch.bfloat16)
+    v = torch.randn((n * Lk, Hkv, D), device=dev, generator=g).to(torch.bfloat16)
+    cq = torch.arange(0, (n + 1) * Lq, Lq, device=dev, dtype=torch.int64)
+    ck = torch.arange(0, (n + 1) * Lk, Lk, device=dev, dtype=torch.int64)
+    o = torch.empty_like(q)
+    lse = torch.empty((Hq, n * Lq), dtype=torch.float32, device=dev)
+    ws = torch.empty(mosaic.attn_workspace_bytes(n, n * Lq, Hq, Hkv, D), dtype=torch.uint8, device=dev)
+    call = lambda: mosaic.agg_prefill_attn_kv(q, k, v, cq, ck, n, Lq, D ** -0.5, o=o, lse=lse,
+                                              workspace=ws)
+    for _ in range(2):
+        call()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in range(3)]
+    torch.cuda.synchronize()
+    for e0, e1 in evs:
+        e0.record()
+        call()
+        e1.record()
+    torch.cuda.synchronize()
+    t = float(np.mean([e0.elapsed_time(e1) for e0, e1 in evs])) * 1e-3
+    pairs = n * sum(float(Lk - Lq + i + 1) for i in range(Lq))
+    fl = 4.0 * Hq * D * pairs
+    return {"workload": "SURVEY 8(f) N2: last 8192 rows of 2 x 32768-token contexts, Hq/Hkv/D=32/8/128",
+            "ms_per_call": t * 1e3, "tflops": fl / t / 1e12,
+            "roofline": {"bound": "tensor", "achieved": fl / t / 1e12, "peak": pk["bf16_tflops"],
+                         "unit": "TFLOP/s", "frac": fl / t / 1e12 / pk["bf16_tflops"], "traffic": None}}
+
+
 def run_product(args):
     import torch
     import torch.distributed as dist
@@ -477,6 +513,7 @@ def run_product(args):
     assemble_info = bench_assemble(torch, mosaic, pk, asm_traffic)
     rope_traffic = (json.loads(tj0.read_text()).get("rope_dram_bytes_per_launch")
                     if tj0.exists() else None)
+    attn_kv_info = bench_attn_kv(torch, mosaic, pk)
     rope_info = bench_rope(torch, mosaic, pk, T, cfg.Hq, cfg.Hkv, cfg.D, rope_traffic)
     f, t, threads, desc = oracle_sample(cfg, 0, args.cpu_rows)
     attn_tflops = flops / (attn_ms * 1e-3) / 1e12
@@ -503,6 +540,7 @@ def run_product(args):
         "gate": gate_info,
         "assemble": assemble_info,
         "rope": rope_info,
+        "attn_kv": attn_kv_info,
         "cpu_baseline": {"value": f / t / 1e12, "unit": UNIT, "cores": threads, "kind": "oracle",
                          "sample": desc},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
