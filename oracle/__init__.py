@@ -115,12 +115,13 @@ def compact(bypass, ctx_len):
                 total_tokens=int(tot[0]), max_seqlen=int(mx[0]))
 
 
-def attn_kv_full(q, k, v, cu_seqlens_q, cu_seqlens_k, softmax_scale):
+def attn_kv_full(q, k, v, cu_seqlens_q, cu_seqlens_k, softmax_scale, causal: bool = True):
     """SURVEY.md 8(f) N2 (prefix-cached / chunked prefill): the q rows of a sequence are the LAST
     Lq of its Lk positions, so row i sees keys j <= i + (Lk - Lq) ("bottom-right" causal alignment,
     DESIGN.md reading N2-1; Lk = Lq is the plain prefill of north_star).  The definition written
     out per (sequence, q head) with numpy in binary64: S = scale Q K^T, mask, row softmax, O = P V,
     LSE = ln sum_j exp(S_ij).  q uint16 [Tq,Hq,D], k/v uint16 [Tk,Hkv,D] (bf16 bits).
+    causal = False: every q row sees all Lk keys (a block of earlier keys in a split-KV prefill).
     Returns (O float64 [Tq,Hq,D], LSE float64 [Hq,Tq])."""
     def f64(bits):
         return (_c(bits, np.uint16).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
@@ -138,8 +139,10 @@ def attn_kv_full(q, k, v, cu_seqlens_q, cu_seqlens_k, softmax_scale):
         Lq, Lk = b - a, d - c
         if Lq == 0:
             continue
-        assert Lk >= Lq
+        assert Lk >= (Lq if causal else 1)
         visible = np.arange(Lk)[None, :] <= (np.arange(Lq)[:, None] + (Lk - Lq))
+        if not causal:
+            visible = np.ones((Lq, Lk), bool)
         for h in range(Hq):
             g = h // (Hq // Hkv)
             S = scale * (Q[a:b, h] @ K[c:d, g].T)
@@ -150,6 +153,21 @@ def attn_kv_full(q, k, v, cu_seqlens_q, cu_seqlens_k, softmax_scale):
             O[a:b, h] = (P / Z) @ V[c:d, g]
             lse[h, a:b] = (M + np.log(Z))[:, 0]
     return O, lse
+
+
+def lse_merge(o_a, lse_a, o_b, lse_b):
+    """the attention result over the union of two disjoint key sets from the
+    partial results over each (binary64): LSE = ln(e^LSE_a + e^LSE_b), O = O_a e^(LSE_a - LSE) +
+    O_b e^(LSE_b - LSE).  o_* float64 [T,Hq,D], lse_* float64 [Hq,T]; -inf = empty partial."""
+    o_a, o_b = np.asarray(o_a, np.float64), np.asarray(o_b, np.float64)
+    la, lb = np.asarray(lse_a, np.float64), np.asarray(lse_b, np.float64)
+    lse = np.logaddexp(la, lb)
+    with np.errstate(invalid="ignore"):
+        wa = np.where(np.isneginf(la), 0.0, np.exp(la - lse))
+        wb = np.where(np.isneginf(lb), 0.0, np.exp(lb - lse))
+    o = np.where(wa.T[:, :, None] != 0, o_a * wa.T[:, :, None], 0.0) + \
+        np.where(wb.T[:, :, None] != 0, o_b * wb.T[:, :, None], 0.0)
+    return o, lse
 
 
 def assemble_context(survivor_idx, cu_seqlens, prompt_tokens, prompt_off, trace_tokens, trace_off,

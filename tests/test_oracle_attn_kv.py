@@ -52,3 +52,33 @@ def test_single_query_identical_keys_closed_form():
     assert np.abs(O[0, 0] - f(v)[:, 0].mean(axis=0)).max() < 1e-12
     dots = np.float64(np.float32(0.2)) * (f(q)[0] * f(krow)[0, 0][None, :]).sum(-1)
     assert np.abs(l[:, 0] - (dots + np.log(Lk))).max() < 1e-12
+
+
+def test_non_causal_rows_see_every_key():
+    """causal = False pinned two ways: the LAST row of the causal problem sees every key, so it
+    must equal the same row of the non-causal one; with identical keys every row is mean(V)."""
+    Lq, Lk, Hq, Hkv, D = 5, 40, 2, 2, 64
+    q, k, v = _bits((Lq, Hq, D), 11), _bits((Lk, Hkv, D), 12), _bits((Lk, Hkv, D), 13)
+    Oc, lc = oracle.attn_kv_full(q, k, v, _cu([Lq]), _cu([Lk]), 0.3, causal=True)
+    On, ln = oracle.attn_kv_full(q, k, v, _cu([Lq]), _cu([Lk]), 0.3, causal=False)
+    assert np.abs(Oc[-1] - On[-1]).max() < 1e-12 and np.abs(lc[:, -1] - ln[:, -1]).max() < 1e-12
+    assert np.abs(Oc[0] - On[0]).max() > 1e-3          # the first row does differ
+    kk = np.repeat(_bits((1, Hkv, D), 14), Lk, axis=0)
+    On, _ = oracle.attn_kv_full(q, kk, v, _cu([Lq]), _cu([Lk]), 0.3, causal=False)
+    f = lambda b: (b.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+    assert np.abs(On[:, 0] - f(v)[:, 0].mean(axis=0)[None, :]).max() < 1e-12
+
+
+def test_merge_of_a_key_split_is_the_unsplit_attention():
+    """oracle.lse_merge pinned to the attention oracle: keys [0, a) seen by all rows >= a, merged with
+    the causal prefill over keys [a, L), must reproduce rows a.. of the plain prefill over [0, L);
+    an empty partial (LSE = -inf) must leave the other unchanged."""
+    L, a, Hq, Hkv, D = 150, 70, 4, 2, 64
+    q, k, v = _bits((L, Hq, D), 21), _bits((L, Hkv, D), 22), _bits((L, Hkv, D), 23)
+    Of, lf = oracle.attn_full(q, k, v, _cu([L]), 0.2)
+    O1, l1 = oracle.attn_kv_full(q[a:], k[:a], v[:a], _cu([L - a]), _cu([a]), 0.2, causal=False)
+    O2, l2 = oracle.attn_full(q[a:], k[a:], v[a:], _cu([L - a]), 0.2)
+    O, l = oracle.lse_merge(O1, l1, O2, l2)
+    assert np.abs(O - Of[a:]).max() < 1e-12 and np.abs(l - lf[:, a:]).max() < 1e-12
+    O, l = oracle.lse_merge(np.full_like(O2, np.nan), np.full_like(l2, -np.inf), O2, l2)
+    assert np.array_equal(O, O2) and np.array_equal(l, l2)
