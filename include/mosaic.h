@@ -158,17 +158,35 @@ mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k, const void
  *   cu_seqlens_q, cu_seqlens_k [dev] int64 [n_seqs + 1]; max_seqlen_q >= every Lq;
  *   o [dev] bf16 [total_q_tokens, Hq, D]; lse [dev] fp32 [Hq, total_q_tokens];
  *   workspace >= mosaic_agg_prefill_attn_workspace_bytes(n_seqs, total_q_tokens, ...).
- * Everything else (alignment, D, errors, asynchrony) as mosaic_agg_prefill_attn.  Lk < Lq is not
- * checked and not supported.
+ *   causal: 1 as above; 0: every q row sees ALL Lk keys of its sequence (the partial result of a
+ *   block of earlier keys in a split-KV prefill; Lk >= 1 wherever Lq >= 1) -- see mosaic_lse_merge.
+ * Everything else (alignment, D, errors, asynchrony) as mosaic_agg_prefill_attn.  Lk < Lq with
+ * causal = 1 is not checked and not supported.
  * ------------------------------------------------------------------------------------------- */
 mosaic_status_t mosaic_agg_prefill_attn_kv(const void* q, const void* k, const void* v,
                                            const int64_t* cu_seqlens_q,
                                            const int64_t* cu_seqlens_k, int32_t n_seqs,
                                            int64_t total_q_tokens, int64_t total_k_tokens,
                                            int32_t max_seqlen_q, int32_t Hq, int32_t Hkv, int32_t D,
-                                           float softmax_scale, void* o, float* lse,
+                                           float softmax_scale, int32_t causal, void* o, float* lse,
                                            void* workspace, size_t workspace_bytes,
                                            void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * mosaic_lse_merge -- SURVEY.md section 8(f) N2: merges the partial attention results of two
+ * DISJOINT key sets A, B for the same q rows (split-KV / chunked prefill):
+ *     LSE = ln(e^LSE_a + e^LSE_b),   O = O_a e^(LSE_a - LSE) + O_b e^(LSE_b - LSE).
+ * This is exact: a row's softmax weights over A u B are its weights over A times e^(LSE_a - LSE)
+ * (north_star's LSE is exported for this).  LSE = -inf marks an empty partial (weight 0; its O
+ * is not read as a number).
+ *
+ *   o_a, o_b [dev] bf16 [total_tokens, Hq, D] (16-byte aligned), lse_a, lse_b [dev] fp32
+ *   [Hq, total_tokens];  o, lse: outputs of the same shapes (o may alias o_a or o_b, lse may alias
+ *   lse_a or lse_b).  D a multiple of 8.  fp32 arithmetic, O rounded to nearest-even bf16.
+ * ------------------------------------------------------------------------------------------- */
+mosaic_status_t mosaic_lse_merge(const void* o_a, const float* lse_a, const void* o_b,
+                                 const float* lse_b, int64_t total_tokens, int32_t Hq, int32_t D,
+                                 void* o, float* lse, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
  * mosaic_assemble_context -- SURVEY.md section 8(f) N1 (a "next" row, between G5 and A1): the

@@ -193,6 +193,7 @@ struct AttnParams {
     int Hq, Hkv;
     float scale_log2;  // |softmax_scale| * log2(e); a negative scale negates Q inside the MMA
     float inv_group;   // 1 / (Hq / Hkv)
+    int causal;        // 0: every q row sees all the keys of its sequence
     int o_align32;     // o is 32-byte aligned: the epilogue may use 256-bit stores
 };
 
@@ -234,7 +235,9 @@ struct Work {
     int64_t t0;      // first q token of the sequence
     int64_t tk0;     // first k token of the sequence
     int L;           // q rows of the sequence
-    int off;         // k length - q length: row i sees keys j <= i + off (0 for plain prefill)
+    int off;         // row i sees keys j <= min(i + off, lk - 1): k length - q length when causal
+                     // (0 for the plain prefill), huge when not
+    int lk;          // keys of the sequence
     int row0;        // first row of the block inside the sequence
     int n0, n1;      // KV tiles of tile 0 / tile 1 (0 = tile has no rows)
     int n_kv;        // max of the two
@@ -261,10 +264,12 @@ __device__ __forceinline__ Work make_work(const AttnParams& p, const int4 it, in
     k.t0 = it.x;
     k.tk0 = it.w;
     k.L = it.y;
-    k.off = lk - it.y;
+    k.off = p.causal ? lk - it.y : (1 << 29);
+    k.lk = lk;
     k.row0 = it.z * BQ;
     // KV tiles of a q tile: up to the last key its last row sees (2c+1 and 2c+2 when off = 0)
-    const int last0 = min(k.row0 + BM, k.L) + k.off, last1 = min(k.row0 + BQ, k.L) + k.off;
+    const int last0 = min(min(k.row0 + BM, k.L) + k.off, lk);
+    const int last1 = min(min(k.row0 + BQ, k.L) + k.off, lk);
     k.n0 = (last0 + BN - 1) / BN;
     k.n1 = (k.row0 + BM < k.L) ? (last1 + BN - 1) / BN : 0;
     k.n_kv = max(k.n0, k.n1);
@@ -792,7 +797,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             // thr >= 63).  With off = 0 these are the two steps of the diagonal tile: untouched for
             // rows 64-127 at b = 0, masked altogether for rows 0-63 at b = 1, partly masked otherwise.
             const int tile_row0 = k.row0 + k.tile_of(t) * BM;  // first row of the tile in the sequence
-            const int u_masked = ((tile_row0 + k.off + 1) >> 6) & ~1;
+            const int u_masked = ((min(tile_row0 + k.off, k.lk - 1) + 1) >> 6) & ~1;
             const int U = 2 * n_t;
             for (int u = 0; u < u_masked; u += 2) {
                 step(M0{}, 0, u == 0);
@@ -801,8 +806,8 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             }
             for (int u = u_masked; u < U; ++u) {
                 const int b = u & 1;
-                thr = tile_row0 + row + k.off - u * BS;
-                if (tile_row0 + wq * 32 + 31 + k.off - u * BS < 0)
+                thr = min(tile_row0 + row + k.off, k.lk - 1) - u * BS;
+                if (min(tile_row0 + wq * 32 + 31 + k.off, k.lk - 1) - u * BS < 0)
                     step(M2{}, b, false);
                 else
                     step(M1{}, b, u == 0);
@@ -894,8 +899,8 @@ namespace {
 mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int64_t* cu_seqlens,
                           const int64_t* cu_seqlens_k, int32_t n_seqs, int64_t total_tokens,
                           int64_t total_k_tokens, int32_t max_seqlen, int32_t Hq, int32_t Hkv,
-                          int32_t D, float softmax_scale, void* o, float* lse, void* workspace,
-                          size_t workspace_bytes, void* cuda_stream) {
+                          int32_t D, float softmax_scale, int causal, void* o, float* lse,
+                          void* workspace, size_t workspace_bytes, void* cuda_stream) {
     if (n_seqs < 0 || total_tokens < 0 || total_tokens >= (1ll << 31) || total_k_tokens < 0 ||
         total_k_tokens >= (1ll << 31) || max_seqlen < 0 || Hq < 1 || Hkv < 1 || Hq % Hkv != 0 ||
         !isfinite(softmax_scale))
@@ -934,6 +939,7 @@ mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int
     p.Hkv = Hkv;
     p.scale_log2 = fabsf(softmax_scale) * kLog2e;
     p.inv_group = 1.0f / (float)(Hq / Hkv);
+    p.causal = causal ? 1 : 0;
     p.o_align32 = (reinterpret_cast<uintptr_t>(o) & 31u) == 0 ? 1 : 0;
     const int negate_q = softmax_scale < 0.f ? 1 : 0;
     const int64_t max_work = (total_tokens / BQ + n_seqs) * (int64_t)Hq;
@@ -952,15 +958,15 @@ extern "C" mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k,
                                                    void* workspace, size_t workspace_bytes,
                                                    void* cuda_stream) {
     return attn_impl(q, k, v, cu_seqlens, cu_seqlens, n_seqs, total_tokens, total_tokens, max_seqlen,
-                     Hq, Hkv, D, softmax_scale, o, lse, workspace, workspace_bytes, cuda_stream);
+                     Hq, Hkv, D, softmax_scale, 1, o, lse, workspace, workspace_bytes, cuda_stream);
 }
 
 extern "C" mosaic_status_t mosaic_agg_prefill_attn_kv(
     const void* q, const void* k, const void* v, const int64_t* cu_seqlens_q,
     const int64_t* cu_seqlens_k, int32_t n_seqs, int64_t total_q_tokens, int64_t total_k_tokens,
-    int32_t max_seqlen_q, int32_t Hq, int32_t Hkv, int32_t D, float softmax_scale, void* o,
-    float* lse, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    int32_t max_seqlen_q, int32_t Hq, int32_t Hkv, int32_t D, float softmax_scale, int32_t causal,
+    void* o, float* lse, void* workspace, size_t workspace_bytes, void* cuda_stream) {
     return attn_impl(q, k, v, cu_seqlens_q, cu_seqlens_k, n_seqs, total_q_tokens, total_k_tokens,
-                     max_seqlen_q, Hq, Hkv, D, softmax_scale, o, lse, workspace, workspace_bytes,
-                     cuda_stream);
+                     max_seqlen_q, Hq, Hkv, D, softmax_scale, causal, o, lse, workspace,
+                     workspace_bytes, cuda_stream);
 }

@@ -1,0 +1,83 @@
+// merge.cu -- SURVEY.md section 8(f) N2: merging the partial attention results of two disjoint
+// key sets for the same q rows (split-KV / chunked prefill of the aggregator's long contexts).
+// With (O_a, LSE_a) over keys A and (O_b, LSE_b) over keys B, the result over A u B is
+//     LSE = ln(e^LSE_a + e^LSE_b),   O = O_a e^(LSE_a - LSE) + O_b e^(LSE_b - LSE)
+// (the softmax weights of a row over A u B are those over A scaled by e^(LSE_a - LSE), and likewise
+// for B).  LSE = -inf marks an empty partial (weight 0).
+//
+// HBM-bound elementwise: a thread takes 8 consecutive elements of one (token, head) row: two
+// 16-byte loads, fp32 math, one 16-byte store; the thread of a row's first chunk writes its LSE.
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include "common.cuh"
+
+namespace mosaic {
+namespace {
+
+constexpr int kMergeThreads = 256;
+
+__global__ void __launch_bounds__(kMergeThreads) lse_merge_kernel(
+    const __nv_bfloat16* __restrict__ oa, const float* __restrict__ la,
+    const __nv_bfloat16* __restrict__ ob, const float* __restrict__ lb, int64_t T, int Hq, int D,
+    __nv_bfloat16* __restrict__ o, float* __restrict__ lse) {
+    const int per_row = D / 8;
+    const int64_t gid = (int64_t)blockIdx.x * kMergeThreads + threadIdx.x;
+    const int64_t rowi = gid / per_row;  // (token, head) row
+    if (rowi >= T * Hq) return;
+    const int c = (int)(gid - rowi * per_row);
+    const int64_t t = rowi / Hq;
+    const int h = (int)(rowi - t * Hq);
+    const float xa = la[(int64_t)h * T + t], xb = lb[(int64_t)h * T + t];
+    const float m = fmaxf(xa, xb);
+    float wa = 0.f, wb = 0.f, out_lse = -INFINITY;
+    if (m > -INFINITY) {
+        const float ea = expf(xa - m), eb = expf(xb - m);  // exp(-inf) = 0 for an empty partial
+        const float z = ea + eb;
+        wa = ea / z;
+        wb = eb / z;
+        out_lse = m + logf(z);
+    }
+    const uint4 va = *reinterpret_cast<const uint4*>(oa + rowi * D + c * 8);
+    const uint4 vb = *reinterpret_cast<const uint4*>(ob + rowi * D + c * 8);
+    const __nv_bfloat162* pa = reinterpret_cast<const __nv_bfloat162*>(&va);
+    const __nv_bfloat162* pb = reinterpret_cast<const __nv_bfloat162*>(&vb);
+    uint4 vo;
+    __nv_bfloat162* po = reinterpret_cast<__nv_bfloat162*>(&vo);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const float2 a = __bfloat1622float2(pa[u]), b = __bfloat1622float2(pb[u]);
+        // (a weight of exactly 0 must not turn an uninitialised partial into NaN)
+        const float x = (wa != 0.f ? a.x * wa : 0.f) + (wb != 0.f ? b.x * wb : 0.f);
+        const float y = (wa != 0.f ? a.y * wa : 0.f) + (wb != 0.f ? b.y * wb : 0.f);
+        po[u] = __floats2bfloat162_rn(x, y);
+    }
+    *reinterpret_cast<uint4*>(o + rowi * D + c * 8) = vo;
+    if (c == 0) lse[(int64_t)h * T + t] = out_lse;
+}
+
+}  // namespace
+}  // namespace mosaic
+
+using namespace mosaic;
+
+extern "C" mosaic_status_t mosaic_lse_merge(const void* o_a, const float* lse_a, const void* o_b,
+                                            const float* lse_b, int64_t total_tokens, int32_t Hq,
+                                            int32_t D, void* o, float* lse, void* cuda_stream) {
+    if (total_tokens < 0 || Hq < 1 || D < 8 || D % 8 != 0) return MOSAIC_ERR_INVALID_ARG;
+    if (total_tokens == 0) return MOSAIC_OK;
+    if (!o_a || !o_b || !lse_a || !lse_b || !o || !lse || !aligned16(o_a) || !aligned16(o_b) ||
+        !aligned16(o))
+        return MOSAIC_ERR_INVALID_ARG;
+    const int64_t threads = total_tokens * Hq * (D / 8);
+    const int64_t blocks = (threads + kMergeThreads - 1) / kMergeThreads;
+    if (blocks >= (1ll << 31)) return MOSAIC_ERR_UNSUPPORTED;
+    lse_merge_kernel<<<(unsigned)blocks, kMergeThreads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        static_cast<const __nv_bfloat16*>(o_a), lse_a, static_cast<const __nv_bfloat16*>(o_b), lse_b,
+        total_tokens, Hq, D, static_cast<__nv_bfloat16*>(o), lse);
+    count_launch();
+    MOSAIC_CUDA_TRY(cudaGetLastError());
+    return MOSAIC_OK;
+}

@@ -31,7 +31,9 @@ SIGNATURES = {
     "mosaic_agg_prefill_attn": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i64, _i32, _i32, _i32,
                                                _i32, _f32, _vp, _vp, _vp, _sz, _vp]),
     "mosaic_agg_prefill_attn_kv": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _i32, _i64, _i64, _i32,
-                                                  _i32, _i32, _i32, _f32, _vp, _vp, _vp, _sz, _vp]),
+                                                  _i32, _i32, _i32, _f32, _i32, _vp, _vp, _vp, _sz,
+                                                  _vp]),
+    "mosaic_lse_merge": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i64, _i32, _i32, _vp, _vp, _vp]),
     "mosaic_assemble_context": (ctypes.c_int, [_vp, _vp, _i32, _i32, _vp, _vp, _vp, _vp, _i32, _vp,
                                                _vp, _vp, _vp]),
     "mosaic_rope_packed": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _i32, _i32, _f32, _vp]),
@@ -203,7 +205,7 @@ def agg_prefill_attn(q, k, v, cu_seqlens, n_seqs, max_seqlen, softmax_scale, *, 
 
 
 def agg_prefill_attn_kv(q, k, v, cu_seqlens_q, cu_seqlens_k, n_seqs, max_seqlen_q, softmax_scale, *,
-                        o=None, lse=None, workspace=None, stream=None):
+                        causal=True, o=None, lse=None, workspace=None, stream=None):
     """mosaic_agg_prefill_attn_kv: q bf16 [Tq,Hq,D], k/v bf16 [Tk,Hkv,D],
     row i of a sequence sees keys j <= i + (Lk - Lq).  Returns (o bf16 [Tq,Hq,D], lse fp32 [Hq,Tq])."""
     Tq, Hq, D = q.shape
@@ -222,9 +224,24 @@ def agg_prefill_attn_kv(q, k, v, cu_seqlens_q, cu_seqlens_k, n_seqs, max_seqlen_
         _dptr(q, torch.bfloat16, "q"), _dptr(k, torch.bfloat16, "k"), _dptr(v, torch.bfloat16, "v"),
         _dptr(cu_seqlens_q, torch.int64, "cu_seqlens_q"), _dptr(cu_seqlens_k, torch.int64, "cu_seqlens_k"),
         int(n_seqs), int(Tq), int(Tk), int(max_seqlen_q), Hq, Hkv, D, float(softmax_scale),
-        _dptr(o, torch.bfloat16, "o"), _dptr(lse, torch.float32, "lse"), _dptr(workspace),
-        workspace.numel(), _stream(stream))
+        1 if causal else 0, _dptr(o, torch.bfloat16, "o"), _dptr(lse, torch.float32, "lse"),
+        _dptr(workspace), workspace.numel(), _stream(stream))
     _check("mosaic_agg_prefill_attn_kv", st)
+    return o, lse
+
+
+def lse_merge(o_a, lse_a, o_b, lse_b, *, o=None, lse=None, stream=None):
+    """mosaic_lse_merge: partial results over two disjoint key sets -> the result over their union."""
+    T, Hq, D = o_a.shape
+    if o is None:
+        o = torch.empty_like(o_a)
+    if lse is None:
+        lse = torch.empty_like(lse_a)
+    st = load().mosaic_lse_merge(_dptr(o_a, torch.bfloat16, "o_a"), _dptr(lse_a, torch.float32, "lse_a"),
+                                 _dptr(o_b, torch.bfloat16, "o_b"), _dptr(lse_b, torch.float32, "lse_b"),
+                                 int(T), Hq, D, _dptr(o, torch.bfloat16, "o"),
+                                 _dptr(lse, torch.float32, "lse"), _stream(stream))
+    _check("mosaic_lse_merge", st)
     return o, lse
 
 

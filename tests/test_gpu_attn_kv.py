@@ -65,3 +65,67 @@ def test_chunked_prefill_of_one_long_sequence():
 def test_sharp_scores_with_offsets():
     eo, el = _case([100, 257], [1124, 300], 2, 1, 128, seed=51, k_scale=8.0)
     assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
+
+
+def test_non_causal_block():
+    """causal = 0: every row sees all keys (ragged Lk: the tail of the last 64-key step is masked
+    by the key count, not by the row)."""
+    Lq, Lk = [1, 130, 64, 300], [1, 77, 640, 1000]
+    cq, ck = _cu(Lq), _cu(Lk)
+    Hq, Hkv, D = 4, 2, 128
+    q = P.randn_bf16((int(cq[-1]), Hq, D), 61)
+    k = P.randn_bf16((int(ck[-1]), Hkv, D), 62)
+    v = P.randn_bf16((int(ck[-1]), Hkv, D), 63)
+    scale = 1.0 / np.sqrt(D)
+    o, lse = mosaic.agg_prefill_attn_kv(q.cuda(), k.cuda(), v.cuda(), torch.from_numpy(cq).cuda(),
+                                        torch.from_numpy(ck).cuda(), len(Lq), max(Lq), scale,
+                                        causal=False)
+    torch.cuda.synchronize()
+    O_ref, lse_ref = oracle.attn_kv_full(P.bf16_bits(q), P.bf16_bits(k), P.bf16_bits(v), cq, ck, scale,
+                                         causal=False)
+    assert np.abs(o.float().cpu().numpy() - O_ref).max() <= P.O_TOL
+    assert np.abs(lse.cpu().numpy() - lse_ref).max() <= P.LSE_TOL
+
+
+def test_split_kv_prefill_merged_on_the_gpu():
+    """A 1 500-token prefill as two key blocks: rows >= a over keys [0, a) (non-causal call), the
+    causal prefill over [a, L), mosaic_lse_merge -- against the plain prefill oracle of the whole."""
+    L, a, Hq, Hkv, D = 1500, 640, 4, 2, 128
+    q, k, v = P.randn_bf16((L, Hq, D), 71), P.randn_bf16((L, Hkv, D), 72), P.randn_bf16((L, Hkv, D), 73)
+    scale = 1.0 / np.sqrt(D)
+    O_ref, lse_ref = oracle.attn_full(P.bf16_bits(q), P.bf16_bits(k), P.bf16_bits(v), _cu([L]), scale)
+    qd, kd, vd = q.cuda(), k.cuda(), v.cuda()
+    n = L - a
+    cu_n = torch.tensor([0, n]).cuda()
+    o1, l1 = mosaic.agg_prefill_attn_kv(qd[a:].contiguous(), kd[:a].contiguous(), vd[:a].contiguous(),
+                                        cu_n, torch.tensor([0, a]).cuda(), 1, n, scale, causal=False)
+    o2, l2 = mosaic.agg_prefill_attn(qd[a:].contiguous(), kd[a:].contiguous(), vd[a:].contiguous(),
+                                     cu_n, 1, n, scale)
+    o, lse = mosaic.lse_merge(o1, l1, o2, l2)
+    torch.cuda.synchronize()
+    # two bf16 roundings of O (the partials, then the merge) instead of one
+    assert np.abs(o.float().cpu().numpy() - O_ref[a:]).max() <= 1.5 * P.O_TOL
+    assert np.abs(lse.cpu().numpy() - lse_ref[:, a:]).max() <= P.LSE_TOL
+
+
+def test_merge_against_the_oracle_and_empty_partials():
+    T, Hq, D = 333, 3, 64
+    g = torch.Generator().manual_seed(81)
+    oa = torch.randn((T, Hq, D), generator=g).to(torch.bfloat16)
+    ob = torch.randn((T, Hq, D), generator=g).to(torch.bfloat16)
+    la = torch.randn((Hq, T), generator=g) * 3
+    lb = torch.randn((Hq, T), generator=g) * 3
+    la[0, :7] = float("-inf")
+    lb[1, 5:9] = float("-inf")
+    la[2, 100], lb[2, 100] = float("-inf"), float("-inf")
+    o, lse = mosaic.lse_merge(oa.cuda(), la.cuda(), ob.cuda(), lb.cuda())
+    torch.cuda.synchronize()
+    O_ref, l_ref = oracle.lse_merge(oa.double().numpy(), la.double().numpy(), ob.double().numpy(),
+                                    lb.double().numpy())
+    got = o.float().cpu().numpy()
+    assert np.all(np.isfinite(got))
+    assert np.abs(got - O_ref).max() <= 2.0 ** -7 * max(1.0, np.abs(O_ref).max())   # one bf16 rounding
+    lg = lse.cpu().numpy()
+    fin = np.isfinite(l_ref)
+    assert np.array_equal(np.isneginf(lg), np.isneginf(l_ref))
+    assert np.abs(lg[fin] - l_ref[fin]).max() <= 1e-5 * (1 + np.abs(l_ref[fin]).max())
