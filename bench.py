@@ -399,6 +399,35 @@ def bench_attn_kv(torch, mosaic, pk):
                          "unit": "TFLOP/s", "frac": fl / t / 1e12 / pk["bf16_tflops"], "traffic": None}}
 
 
+def bench_lse_merge(torch, mosaic, pk, T, Hq, D):
+    """mosaic_lse_merge on two partial results of the bench config's shape.
+    Algorithmic bytes: two bf16 reads and one write per element of O, three fp32 LSE values per row."""
+    dev = "cuda"
+    g = torch.Generator(device=dev).manual_seed(61)
+    oa = torch.randn((T, Hq, D), device=dev, generator=g).to(torch.bfloat16)
+    ob = torch.randn((T, Hq, D), device=dev, generator=g).to(torch.bfloat16)
+    la = torch.randn((Hq, T), device=dev, generator=g)
+    lb = torch.randn((Hq, T), device=dev, generator=g)
+    o, lse = torch.empty_like(oa), torch.empty_like(la)
+    for _ in range(2):
+        mosaic.lse_merge(oa, la, ob, lb, o=o, lse=lse)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in range(5)]
+    torch.cuda.synchronize()
+    for e0, e1 in evs:   # 3.4 GB per call: L2-cold
+        e0.record()
+        mosaic.lse_merge(oa, la, ob, lb, o=o, lse=lse)
+        e1.record()
+    torch.cuda.synchronize()
+    t = float(np.mean([e0.elapsed_time(e1) for e0, e1 in evs])) * 1e-3
+    byts = 6.0 * T * Hq * D + 12.0 * T * Hq
+    return {"workload": "SURVEY 8(f) N2: LSE merge of two partials, T=%d, Hq/D=%d/%d" % (T, Hq, D),
+            "us_per_call": t * 1e6,
+            "roofline": {"bound": "hbm", "achieved": byts / t / 1e9, "peak": pk["hbm_gbs"],
+                         "unit": "GB/s", "frac": byts / t / 1e9 / pk["hbm_gbs"], "traffic": None,
+                         "algorithmic_bytes": byts}}
+
+
 def run_product(args):
     import torch
     import torch.distributed as dist
@@ -514,6 +543,7 @@ def run_product(args):
     rope_traffic = (json.loads(tj0.read_text()).get("rope_dram_bytes_per_launch")
                     if tj0.exists() else None)
     attn_kv_info = bench_attn_kv(torch, mosaic, pk)
+    merge_info = bench_lse_merge(torch, mosaic, pk, T, cfg.Hq, cfg.D)
     rope_info = bench_rope(torch, mosaic, pk, T, cfg.Hq, cfg.Hkv, cfg.D, rope_traffic)
     f, t, threads, desc = oracle_sample(cfg, 0, args.cpu_rows)
     attn_tflops = flops / (attn_ms * 1e-3) / 1e12
@@ -541,6 +571,7 @@ def run_product(args):
         "assemble": assemble_info,
         "rope": rope_info,
         "attn_kv": attn_kv_info,
+        "lse_merge": merge_info,
         "cpu_baseline": {"value": f / t / 1e12, "unit": UNIT, "cores": threads, "kind": "oracle",
                          "sample": desc},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
