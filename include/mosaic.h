@@ -189,6 +189,25 @@ mosaic_status_t mosaic_lse_merge(const void* o_a, const float* lse_a, const void
                                  void* o, float* lse, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * mosaic_agg_decode_attn -- SURVEY.md section 8(f) N2: the aggregator's GQA decode attention, one
+ * new q token per sequence against all Lk cached keys of that sequence (decode follows prefill in
+ * the aggregator): O[s,h,:] = softmax_j(scale q_{s,h} . k_{j,g(h)}) V, LSE as north_star.
+ * K and V are read once: the Hq / Hkv q heads of a KV head go through the prefill kernel together
+ * as the rows of one tile (see decode.cu).
+ *
+ *   q [dev] bf16 [n_seqs, Hq, D]; k, v [dev] bf16 [total_k_tokens, Hkv, D]; cu_seqlens_k [dev]
+ *   int64 [n_seqs + 1] (every Lk >= 1); o [dev] bf16 [n_seqs, Hq, D]; lse [dev] fp32 [Hq, n_seqs];
+ *   workspace [dev] >= mosaic_agg_decode_attn_workspace_bytes(n_seqs, Hq, Hkv, D), 16-byte aligned.
+ * Hq / Hkv <= 128; D, alignment, errors and asynchrony as mosaic_agg_prefill_attn.
+ * ------------------------------------------------------------------------------------------- */
+size_t mosaic_agg_decode_attn_workspace_bytes(int32_t n_seqs, int32_t Hq, int32_t Hkv, int32_t D);
+mosaic_status_t mosaic_agg_decode_attn(const void* q, const void* k, const void* v,
+                                       const int64_t* cu_seqlens_k, int32_t n_seqs,
+                                       int64_t total_k_tokens, int32_t Hq, int32_t Hkv, int32_t D,
+                                       float softmax_scale, void* o, float* lse, void* workspace,
+                                       size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * mosaic_assemble_context -- SURVEY.md section 8(f) N1 (a "next" row, between G5 and A1): the
  * survivors' aggregator contexts as one packed token batch.  The aggregator "process[es] the
  * combined output or reasoning traces of its experts" (Alg. 1

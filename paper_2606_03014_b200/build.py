@@ -14,7 +14,7 @@ CSRC = PKG / "csrc"
 INCLUDE = ROOT / "include"
 LIB = PKG / "libmosaic.so"
 OBJ_DIR = PKG / "build"
-SOURCES = ["core.cu", "gate.cu", "attn.cu", "stage.cu", "assemble.cu", "rope.cu", "merge.cu"]
+SOURCES = ["core.cu", "gate.cu", "attn.cu", "stage.cu", "assemble.cu", "rope.cu", "merge.cu", "decode.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC",
               f"-I{INCLUDE}", f"-I{CSRC}"]

@@ -33,6 +33,9 @@ SIGNATURES = {
     "mosaic_agg_prefill_attn_kv": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _i32, _i64, _i64, _i32,
                                                   _i32, _i32, _i32, _f32, _i32, _vp, _vp, _vp, _sz,
                                                   _vp]),
+    "mosaic_agg_decode_attn_workspace_bytes": (_sz, [_i32, _i32, _i32, _i32]),
+    "mosaic_agg_decode_attn": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i64, _i32, _i32, _i32, _f32,
+                                              _vp, _vp, _vp, _sz, _vp]),
     "mosaic_lse_merge": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i64, _i32, _i32, _vp, _vp, _vp]),
     "mosaic_assemble_context": (ctypes.c_int, [_vp, _vp, _i32, _i32, _vp, _vp, _vp, _vp, _i32, _vp,
                                                _vp, _vp, _vp]),
@@ -227,6 +230,29 @@ def agg_prefill_attn_kv(q, k, v, cu_seqlens_q, cu_seqlens_k, n_seqs, max_seqlen_
         1 if causal else 0, _dptr(o, torch.bfloat16, "o"), _dptr(lse, torch.float32, "lse"),
         _dptr(workspace), workspace.numel(), _stream(stream))
     _check("mosaic_agg_prefill_attn_kv", st)
+    return o, lse
+
+
+def agg_decode_attn(q, k, v, cu_seqlens_k, softmax_scale, *, o=None, lse=None, workspace=None,
+                    stream=None):
+    """mosaic_agg_decode_attn: q bf16 [n_seqs,Hq,D] (one token per sequence) against k/v bf16
+    [Tk,Hkv,D].  Returns (o bf16 [n_seqs,Hq,D], lse fp32 [Hq,n_seqs])."""
+    n, Hq, D = q.shape
+    Tk, Hkv = k.shape[0], k.shape[1]
+    dev = q.device
+    if o is None:
+        o = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty((Hq, n), dtype=torch.float32, device=dev)
+    if workspace is None:
+        nb = int(load().mosaic_agg_decode_attn_workspace_bytes(n, Hq, Hkv, D))
+        workspace = torch.empty(max(nb, 16), dtype=torch.uint8, device=dev)
+    st = load().mosaic_agg_decode_attn(
+        _dptr(q, torch.bfloat16, "q"), _dptr(k, torch.bfloat16, "k"), _dptr(v, torch.bfloat16, "v"),
+        _dptr(cu_seqlens_k, torch.int64, "cu_seqlens_k"), int(n), int(Tk), Hq, Hkv, D,
+        float(softmax_scale), _dptr(o, torch.bfloat16, "o"), _dptr(lse, torch.float32, "lse"),
+        _dptr(workspace), workspace.numel(), _stream(stream))
+    _check("mosaic_agg_decode_attn", st)
     return o, lse
 
 
