@@ -428,6 +428,44 @@ def bench_lse_merge(torch, mosaic, pk, T, Hq, D):
                          "algorithmic_bytes": byts}}
 
 
+def bench_decode(torch, mosaic, pk):
+    """mosaic_agg_decode_attn, one new token for each of 64 sequences of
+    U{8192..32768} cached keys, Hq/Hkv/D = 32/8/128.  Algorithmic bytes: K and V read once."""
+    n, Hq, Hkv, D = 64, 32, 8, 128
+    g = np.random.default_rng(71)
+    Lk = g.integers(8192, 32769, size=n).astype(np.int64)
+    ck = np.concatenate([[0], np.cumsum(Lk)]).astype(np.int64)
+    Tk = int(ck[-1])
+    dev = "cuda"
+    gt = torch.Generator(device=dev).manual_seed(71)
+    q = torch.randn((n, Hq, D), device=dev, generator=gt).to(torch.bfloat16)
+    k = torch.randn((Tk, Hkv, D), device=dev, generator=gt).to(torch.bfloat16)
+    v = torch.randn((Tk, Hkv, D), device=dev, generator=gt).to(torch.bfloat16)
+    ck_d = torch.from_numpy(ck).to(dev)
+    o = torch.empty_like(q)
+    lse = torch.empty((Hq, n), dtype=torch.float32, device=dev)
+    ws = torch.empty(int(mosaic.load().mosaic_agg_decode_attn_workspace_bytes(n, Hq, Hkv, D)),
+                     dtype=torch.uint8, device=dev)
+    call = lambda: mosaic.agg_decode_attn(q, k, v, ck_d, D ** -0.5, o=o, lse=lse, workspace=ws)
+    for _ in range(2):
+        call()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in range(5)]
+    torch.cuda.synchronize()
+    for e0, e1 in evs:   # K + V = 5 GB: L2-cold
+        e0.record()
+        call()
+        e1.record()
+    torch.cuda.synchronize()
+    t = float(np.mean([e0.elapsed_time(e1) for e0, e1 in evs])) * 1e-3
+    byts = 4.0 * Tk * Hkv * D
+    return {"workload": "SURVEY 8(f) N2: decode, 64 sequences of U{8192..32768} keys, Hq/Hkv/D=32/8/128",
+            "cached_tokens": Tk, "us_per_call": t * 1e6,
+            "roofline": {"bound": "hbm", "achieved": byts / t / 1e9, "peak": pk["hbm_gbs"],
+                         "unit": "GB/s", "frac": byts / t / 1e9 / pk["hbm_gbs"], "traffic": None,
+                         "algorithmic_bytes": byts}}
+
+
 def run_product(args):
     import torch
     import torch.distributed as dist
@@ -543,6 +581,7 @@ def run_product(args):
     rope_traffic = (json.loads(tj0.read_text()).get("rope_dram_bytes_per_launch")
                     if tj0.exists() else None)
     attn_kv_info = bench_attn_kv(torch, mosaic, pk)
+    decode_info = bench_decode(torch, mosaic, pk)
     merge_info = bench_lse_merge(torch, mosaic, pk, T, cfg.Hq, cfg.D)
     rope_info = bench_rope(torch, mosaic, pk, T, cfg.Hq, cfg.Hkv, cfg.D, rope_traffic)
     f, t, threads, desc = oracle_sample(cfg, 0, args.cpu_rows)
@@ -572,6 +611,7 @@ def run_product(args):
         "rope": rope_info,
         "attn_kv": attn_kv_info,
         "lse_merge": merge_info,
+        "decode": decode_info,
         "cpu_baseline": {"value": f / t / 1e12, "unit": UNIT, "cores": threads, "kind": "oracle",
                          "sample": desc},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
