@@ -62,6 +62,29 @@ def test_host_side_validation_needs_no_gpu(lib):
     assert lib.mosaic_agg_prefill_attn(*args(8, 2, 96, 1, 128)) == 2
     assert lib.mosaic_agg_prefill_attn(*args(8, 2, 128, 0, 0)) == 0
     assert lib.mosaic_agg_prefill_attn(*args(8, 2, 128, 1, 1 << 31)) == 1
+    # the SURVEY 8(f) entries validate before they touch the device too
+    kv = lambda Hq, Hkv, D, n, Tq, Tk: (fake, fake, fake, fake, fake, n, Tq, Tk, 128, Hq, Hkv, D, 0.1,
+                                        1, fake, fake, fake, 1 << 20, None)
+    assert lib.mosaic_agg_prefill_attn_kv(*kv(7, 2, 128, 1, 128, 256)) == 1
+    assert lib.mosaic_agg_prefill_attn_kv(*kv(8, 2, 96, 1, 128, 256)) == 2
+    assert lib.mosaic_agg_prefill_attn_kv(*kv(8, 2, 128, 1, 128, 1 << 31)) == 1
+    assert lib.mosaic_agg_prefill_attn_kv(*kv(8, 2, 128, 0, 0, 0)) == 0
+    asm = lambda n, E: (fake, fake, n, 100, fake, fake, fake, fake, E, fake, fake, None, None)
+    assert lib.mosaic_assemble_context(*asm(4, 0)) == 1
+    assert lib.mosaic_assemble_context(*asm(4, 33)) == 1
+    assert lib.mosaic_assemble_context(*asm(-1, 3)) == 1
+    assert lib.mosaic_rope_packed(fake, fake, fake, 16, 4, 2, 96, 1e6, None) == 2
+    assert lib.mosaic_rope_packed(fake, fake, fake, 16, 4, 2, 128, 0.0, None) == 1
+    assert lib.mosaic_rope_packed(fake, fake, fake, 0, 4, 2, 128, 1e6, None) == 0
+    assert lib.mosaic_lse_merge(fake, fake, fake, fake, 16, 4, 100, fake, fake, None) == 1
+    assert lib.mosaic_lse_merge(fake, fake, fake, fake, 0, 4, 128, fake, fake, None) == 0
+    dec = lambda Hq, Hkv, D, n: (fake, fake, fake, fake, n, 1000, Hq, Hkv, D, 0.1, fake, fake, fake,
+                                 1 << 20, None)
+    assert lib.mosaic_agg_decode_attn(*dec(7, 2, 128, 4)) == 1
+    assert lib.mosaic_agg_decode_attn(*dec(8, 2, 96, 4)) == 2
+    assert lib.mosaic_agg_decode_attn(*dec(8, 2, 128, 0)) == 0
+    assert lib.mosaic_agg_decode_attn_workspace_bytes(4, 8, 2, 128) > 0
+    assert lib.mosaic_agg_decode_attn_workspace_bytes(4, 7, 2, 128) == 0
 
 
 def test_product_path_does_not_import_oracle():
