@@ -444,7 +444,7 @@ def bench_decode(torch, mosaic, pk):
     ck_d = torch.from_numpy(ck).to(dev)
     o = torch.empty_like(q)
     lse = torch.empty((Hq, n), dtype=torch.float32, device=dev)
-    ws = torch.empty(int(mosaic.load().mosaic_agg_decode_attn_workspace_bytes(n, Hq, Hkv, D)),
+    ws = torch.empty(int(mosaic.load().mosaic_agg_decode_attn_workspace_bytes(n, Tk, Hq, Hkv, D)),
                      dtype=torch.uint8, device=dev)
     call = lambda: mosaic.agg_decode_attn(q, k, v, ck_d, D ** -0.5, o=o, lse=lse, workspace=ws)
     for _ in range(2):

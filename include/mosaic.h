@@ -193,14 +193,18 @@ mosaic_status_t mosaic_lse_merge(const void* o_a, const float* lse_a, const void
  * new q token per sequence against all Lk cached keys of that sequence (decode follows prefill in
  * the aggregator): O[s,h,:] = softmax_j(scale q_{s,h} . k_{j,g(h)}) V, LSE as north_star.
  * K and V are read once: the Hq / Hkv q heads of a KV head go through the prefill kernel together
- * as the rows of one tile (see decode.cu).
+ * as the rows of one tile, and every sequence's keys are cut into chunks whose partial results
+ * are merged by their LSEs, so that a few long sequences still fill the GPU (see decode.cu).
+ * A sequence without keys gets O = 0 and LSE = -inf.
  *
  *   q [dev] bf16 [n_seqs, Hq, D]; k, v [dev] bf16 [total_k_tokens, Hkv, D]; cu_seqlens_k [dev]
- *   int64 [n_seqs + 1] (every Lk >= 1); o [dev] bf16 [n_seqs, Hq, D]; lse [dev] fp32 [Hq, n_seqs];
- *   workspace [dev] >= mosaic_agg_decode_attn_workspace_bytes(n_seqs, Hq, Hkv, D), 16-byte aligned.
+ *   int64 [n_seqs + 1]; o [dev] bf16 [n_seqs, Hq, D]; lse [dev] fp32 [Hq, n_seqs];
+ *   workspace [dev] >= mosaic_agg_decode_attn_workspace_bytes(n_seqs, total_k_tokens, Hq, Hkv, D),
+ *   16-byte aligned.
  * Hq / Hkv <= 128; D, alignment, errors and asynchrony as mosaic_agg_prefill_attn.
  * ------------------------------------------------------------------------------------------- */
-size_t mosaic_agg_decode_attn_workspace_bytes(int32_t n_seqs, int32_t Hq, int32_t Hkv, int32_t D);
+size_t mosaic_agg_decode_attn_workspace_bytes(int32_t n_seqs, int64_t total_k_tokens, int32_t Hq,
+                                              int32_t Hkv, int32_t D);
 mosaic_status_t mosaic_agg_decode_attn(const void* q, const void* k, const void* v,
                                        const int64_t* cu_seqlens_k, int32_t n_seqs,
                                        int64_t total_k_tokens, int32_t Hq, int32_t Hkv, int32_t D,

@@ -33,7 +33,7 @@ SIGNATURES = {
     "mosaic_agg_prefill_attn_kv": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _i32, _i64, _i64, _i32,
                                                   _i32, _i32, _i32, _f32, _i32, _vp, _vp, _vp, _sz,
                                                   _vp]),
-    "mosaic_agg_decode_attn_workspace_bytes": (_sz, [_i32, _i32, _i32, _i32]),
+    "mosaic_agg_decode_attn_workspace_bytes": (_sz, [_i32, _i64, _i32, _i32, _i32]),
     "mosaic_agg_decode_attn": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i64, _i32, _i32, _i32, _f32,
                                               _vp, _vp, _vp, _sz, _vp]),
     "mosaic_lse_merge": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i64, _i32, _i32, _vp, _vp, _vp]),
@@ -245,7 +245,7 @@ def agg_decode_attn(q, k, v, cu_seqlens_k, softmax_scale, *, o=None, lse=None, w
     if lse is None:
         lse = torch.empty((Hq, n), dtype=torch.float32, device=dev)
     if workspace is None:
-        nb = int(load().mosaic_agg_decode_attn_workspace_bytes(n, Hq, Hkv, D))
+        nb = int(load().mosaic_agg_decode_attn_workspace_bytes(n, Tk, Hq, Hkv, D))
         workspace = torch.empty(max(nb, 16), dtype=torch.uint8, device=dev)
     st = load().mosaic_agg_decode_attn(
         _dptr(q, torch.bfloat16, "q"), _dptr(k, torch.bfloat16, "k"), _dptr(v, torch.bfloat16, "v"),

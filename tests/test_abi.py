@@ -83,8 +83,8 @@ def test_host_side_validation_needs_no_gpu(lib):
     assert lib.mosaic_agg_decode_attn(*dec(7, 2, 128, 4)) == 1
     assert lib.mosaic_agg_decode_attn(*dec(8, 2, 96, 4)) == 2
     assert lib.mosaic_agg_decode_attn(*dec(8, 2, 128, 0)) == 0
-    assert lib.mosaic_agg_decode_attn_workspace_bytes(4, 8, 2, 128) > 0
-    assert lib.mosaic_agg_decode_attn_workspace_bytes(4, 7, 2, 128) == 0
+    assert lib.mosaic_agg_decode_attn_workspace_bytes(4, 1000, 8, 2, 128) > 0
+    assert lib.mosaic_agg_decode_attn_workspace_bytes(4, 1000, 7, 2, 128) == 0
 
 
 def test_product_path_does_not_import_oracle():

@@ -28,6 +28,28 @@ def test_decode_matches_oracle(D, Hq, Hkv):
     assert np.abs(lse.cpu().numpy() - lse_ref).max() <= P.LSE_TOL
 
 
+def test_decode_few_long_sequences_and_no_keys():
+    """Two long sequences (many chunks each: the split-KV merge) and one without keys (O = 0,
+    LSE = -inf)."""
+    Lk = [9000, 0, 20001]
+    ck = np.concatenate([[0], np.cumsum(Lk)]).astype(np.int64)
+    Hq, Hkv, D = 8, 2, 128
+    q = P.randn_bf16((3, Hq, D), 94)
+    k = P.randn_bf16((int(ck[-1]), Hkv, D), 95)
+    v = P.randn_bf16((int(ck[-1]), Hkv, D), 96)
+    scale = 1.0 / np.sqrt(D)
+    o, lse = mosaic.agg_decode_attn(q.cuda(), k.cuda(), v.cuda(), torch.from_numpy(ck).cuda(), scale)
+    torch.cuda.synchronize()
+    keep = [0, 2]
+    ck2 = np.concatenate([[0], np.cumsum([Lk[i] for i in keep])]).astype(np.int64)
+    O_ref, lse_ref = oracle.attn_kv_full(P.bf16_bits(q[keep]), P.bf16_bits(k), P.bf16_bits(v),
+                                         np.arange(3, dtype=np.int64), ck2, scale)
+    og, lg = o.float().cpu().numpy(), lse.cpu().numpy()
+    assert np.abs(og[keep] - O_ref).max() <= P.O_TOL
+    assert np.abs(lg[:, keep] - lse_ref).max() <= P.LSE_TOL
+    assert np.all(og[1] == 0) and np.all(np.isneginf(lg[:, 1]))
+
+
 def test_decode_empty_batch():
     q = torch.empty((0, 4, 64), dtype=torch.bfloat16, device="cuda")
     k = torch.zeros((8, 2, 64), dtype=torch.bfloat16, device="cuda")
