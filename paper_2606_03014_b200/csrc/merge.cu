@@ -23,7 +23,10 @@ __global__ void __launch_bounds__(kMergeThreads) lse_merge_kernel(
     const __nv_bfloat16* __restrict__ oa, const float* __restrict__ la,
     const __nv_bfloat16* __restrict__ ob, const float* __restrict__ lb, int64_t T, int Hq, int D,
     __nv_bfloat16* __restrict__ o, float* __restrict__ lse) {
-    const int per_row = D / 8;
+    // two 8-element chunks of a row per thread when the row has an even number of them: the row's
+    // LSE pair and weights are computed once for both, and four loads are in flight
+    const int n_sub = (D % 16 == 0) ? 2 : 1;
+    const int per_row = D / (8 * n_sub);
     const int64_t gid = (int64_t)blockIdx.x * kMergeThreads + threadIdx.x;
     const int64_t rowi = gid / per_row;  // (token, head) row
     if (rowi >= T * Hq) return;
@@ -31,6 +34,14 @@ __global__ void __launch_bounds__(kMergeThreads) lse_merge_kernel(
     const int64_t t = rowi / Hq;
     const int h = (int)(rowi - t * Hq);
     const float xa = la[(int64_t)h * T + t], xb = lb[(int64_t)h * T + t];
+    uint4 va[2], vb[2];
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+        if (u < n_sub) {
+            va[u] = *reinterpret_cast<const uint4*>(oa + rowi * D + (c + u * per_row) * 8);
+            vb[u] = *reinterpret_cast<const uint4*>(ob + rowi * D + (c + u * per_row) * 8);
+        }
+    }
     const float m = fmaxf(xa, xb);
     float wa = 0.f, wb = 0.f, out_lse = -INFINITY;
     if (m > -INFINITY) {
@@ -40,21 +51,24 @@ __global__ void __launch_bounds__(kMergeThreads) lse_merge_kernel(
         wb = eb / z;
         out_lse = m + logf(z);
     }
-    const uint4 va = *reinterpret_cast<const uint4*>(oa + rowi * D + c * 8);
-    const uint4 vb = *reinterpret_cast<const uint4*>(ob + rowi * D + c * 8);
-    const __nv_bfloat162* pa = reinterpret_cast<const __nv_bfloat162*>(&va);
-    const __nv_bfloat162* pb = reinterpret_cast<const __nv_bfloat162*>(&vb);
-    uint4 vo;
-    __nv_bfloat162* po = reinterpret_cast<__nv_bfloat162*>(&vo);
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-        const float2 a = __bfloat1622float2(pa[u]), b = __bfloat1622float2(pb[u]);
-        // (a weight of exactly 0 must not turn an uninitialised partial into NaN)
-        const float x = (wa != 0.f ? a.x * wa : 0.f) + (wb != 0.f ? b.x * wb : 0.f);
-        const float y = (wa != 0.f ? a.y * wa : 0.f) + (wb != 0.f ? b.y * wb : 0.f);
-        po[u] = __floats2bfloat162_rn(x, y);
+    for (int u = 0; u < 2; ++u) {
+        if (u < n_sub) {
+            const __nv_bfloat162* pa = reinterpret_cast<const __nv_bfloat162*>(&va[u]);
+            const __nv_bfloat162* pb = reinterpret_cast<const __nv_bfloat162*>(&vb[u]);
+            uint4 vo;
+            __nv_bfloat162* po = reinterpret_cast<__nv_bfloat162*>(&vo);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const float2 a = __bfloat1622float2(pa[e]), b = __bfloat1622float2(pb[e]);
+                // (a weight of exactly 0 must not turn an uninitialised partial into NaN)
+                const float x = (wa != 0.f ? a.x * wa : 0.f) + (wb != 0.f ? b.x * wb : 0.f);
+                const float y = (wa != 0.f ? a.y * wa : 0.f) + (wb != 0.f ? b.y * wb : 0.f);
+                po[e] = __floats2bfloat162_rn(x, y);
+            }
+            *reinterpret_cast<uint4*>(o + rowi * D + (c + u * per_row) * 8) = vo;
+        }
     }
-    *reinterpret_cast<uint4*>(o + rowi * D + c * 8) = vo;
     if (c == 0) lse[(int64_t)h * T + t] = out_lse;
 }
 
@@ -71,7 +85,7 @@ extern "C" mosaic_status_t mosaic_lse_merge(const void* o_a, const float* lse_a,
     if (!o_a || !o_b || !lse_a || !lse_b || !o || !lse || !aligned16(o_a) || !aligned16(o_b) ||
         !aligned16(o))
         return MOSAIC_ERR_INVALID_ARG;
-    const int64_t threads = total_tokens * Hq * (D / 8);
+    const int64_t threads = total_tokens * Hq * (D % 16 == 0 ? D / 16 : D / 8);
     const int64_t blocks = (threads + kMergeThreads - 1) / kMergeThreads;
     if (blocks >= (1ll << 31)) return MOSAIC_ERR_UNSUPPORTED;
     lse_merge_kernel<<<(unsigned)blocks, kMergeThreads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
