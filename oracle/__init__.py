@@ -95,6 +95,19 @@ def gate(answers, tau, expert_conf=None, conf_mode: int = 0):
     return out
 
 
+def gate_tau_per_query(answers, tau_q, expert_conf=None, conf_mode: int = 0):
+    """the gate with a threshold per question (a per-task tau table gathered by
+    the caller's task ids; the paper names its single static threshold as a limitation).
+    Vote, mode and confidence do not depend on the threshold (Alg. 1 lines 2-3): they are the
+    scalar gate's; line 4 becomes bypass[q] = conf[q] >= tau_q[q], compared in fp32 like reading
+    G-4 compares the scalar.  A NaN threshold never bypasses."""
+    tau_q = _c(tau_q, np.float32)
+    out = gate(answers, 0.0, expert_conf, conf_mode)
+    assert tau_q.shape == out["conf"].shape
+    out["bypass"] = (out["conf"] >= tau_q).astype(np.uint8)
+    return out
+
+
 def compact(bypass, ctx_len):
     """Alg. 1 line 6 survivors as a ragged batch (BJ:north_star).
 
