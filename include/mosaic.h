@@ -146,6 +146,24 @@ mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k, const void
                                         void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * mosaic_gate_compact_tau -- SURVEY.md section 8(f) N3 (a "next" row): mosaic_gate_compact with a
+ * threshold PER QUESTION.  The paper fixes one skip criterion per task in advance and names that
+ * as a limitation (P:L188 invites other criteria); with tau_per_query[q] = table[task(q)]
+ * a mixed batch of tasks is gated in one call.  Alg. 1 line 4 becomes
+ *     bypass[q] = conf[q] >= tau_per_query[q]      (fp32 compare; a NaN threshold never bypasses);
+ * vote, mode and confidence are mosaic_gate's.
+ *   tau_per_query [dev] fp32 [Q]; every other argument as mosaic_gate_compact.
+ * ------------------------------------------------------------------------------------------- */
+mosaic_status_t mosaic_gate_compact_tau(const int32_t* answers, const float* expert_conf,
+                                        const int32_t* ctx_len, int64_t Q, int32_t E,
+                                        const float* tau_per_query, int32_t conf_mode,
+                                        int32_t* mode_out, int32_t* count_out, float* agree_out,
+                                        float* conf_out, uint8_t* bypass_out, int32_t* survivor_idx,
+                                        int64_t* cu_seqlens, int32_t* n_survivors,
+                                        int64_t* total_tokens, int32_t* max_seqlen, void* workspace,
+                                        size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * mosaic_agg_prefill_attn_kv -- SURVEY.md section 8(f) N2 (a "next" row): the same attention with
  * the q rows and the keys of a sequence packed separately, for prefix-cached prompts and chunked
  * prefill of the aggregator's long contexts (32 k-class windows): sequence s has Lq q rows

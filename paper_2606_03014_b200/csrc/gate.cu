@@ -237,6 +237,7 @@ struct GateArgs {
     int64_t Q;
     int32_t E;
     float tau;
+    const float* tau_q;  // a threshold per question, else NULL: tau for all
     int32_t* mode_out;
     int32_t* count_out;
     float* agree_out;
@@ -514,7 +515,8 @@ __global__ void __launch_bounds__(kThreads, kBlocksPerSM) gate_compact_kernel(co
                     int32_t mode, count;
                     float agree, conf;
                     bool bypass;
-                    gate_row<EM, CONF, (E_T != 0)>(a[k], w[k], E, p.tau, mode, count, agree, conf, bypass);
+                    gate_row<EM, CONF, (E_T != 0)>(a[k], w[k], E, p.tau_q ? __ldg(p.tau_q + q) : p.tau, mode,
+                                                   count, agree, conf, bypass);
                     if (p.mode_out) __stcs(p.mode_out + q, mode);
                     if (p.count_out) __stcs(p.count_out + q, count);
                     if (p.agree_out) __stcs(p.agree_out + q, agree);
@@ -738,6 +740,43 @@ extern "C" mosaic_status_t mosaic_gate_compact(
     a.Q = Q;
     a.E = E;
     a.tau = tau;
+    a.mode_out = mode_out;
+    a.count_out = count_out;
+    a.agree_out = agree_out;
+    a.conf_out = conf_out;
+    a.bypass_out = bypass_out;
+    a.survivor_idx = survivor_idx;
+    a.cu_seqlens = cu_seqlens;
+    a.n_survivors = n_survivors;
+    a.total_tokens = total_tokens;
+    a.max_seqlen = max_seqlen;
+    return conf_mode == MOSAIC_CONF_WEIGHTED
+               ? dispatch_gate<MOSAIC_CONF_WEIGHTED, true>(a, workspace_bytes, workspace, s)
+               : dispatch_gate<MOSAIC_CONF_VOTE, true>(a, workspace_bytes, workspace, s);
+}
+
+extern "C" mosaic_status_t mosaic_gate_compact_tau(
+    const int32_t* answers, const float* expert_conf, const int32_t* ctx_len, int64_t Q, int32_t E,
+    const float* tau_per_query, int32_t conf_mode, int32_t* mode_out, int32_t* count_out, float* agree_out,
+    float* conf_out, uint8_t* bypass_out, int32_t* survivor_idx, int64_t* cu_seqlens,
+    int32_t* n_survivors, int64_t* total_tokens, int32_t* max_seqlen, void* workspace,
+    size_t workspace_bytes, void* cuda_stream) {
+    mosaic_status_t st = check_gate_args(answers, expert_conf, Q, E, 0.5f, conf_mode);
+    if (st == MOSAIC_OK && Q > 0 && !tau_per_query) st = MOSAIC_ERR_INVALID_ARG;
+    if (st != MOSAIC_OK) return st;
+    if (!cu_seqlens || !n_survivors || !total_tokens || !max_seqlen) return MOSAIC_ERR_INVALID_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    if (Q == 0) return write_empty_batch(cu_seqlens, n_survivors, total_tokens, max_seqlen, s);
+    if (!ctx_len || !survivor_idx || !workspace || !aligned16(workspace))
+        return MOSAIC_ERR_INVALID_ARG;
+    GateArgs a{};
+    a.answers = answers;
+    a.expert_conf = expert_conf;
+    a.ctx_len = ctx_len;
+    a.Q = Q;
+    a.E = E;
+    a.tau = 0.f;
+    a.tau_q = tau_per_query;
     a.mode_out = mode_out;
     a.count_out = count_out;
     a.agree_out = agree_out;

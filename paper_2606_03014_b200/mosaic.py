@@ -27,6 +27,8 @@ SIGNATURES = {
     "mosaic_compact": (ctypes.c_int, [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     "mosaic_gate_compact": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _f32, _i32, _vp, _vp, _vp,
                                            _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "mosaic_gate_compact_tau": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _vp, _i32, _vp, _vp, _vp,
+                                               _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     "mosaic_agg_prefill_attn_workspace_bytes": (_sz, [_i32, _i64, _i32, _i32, _i32]),
     "mosaic_agg_prefill_attn": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i64, _i32, _i32, _i32,
                                                _i32, _f32, _vp, _vp, _vp, _sz, _vp]),
@@ -175,6 +177,27 @@ def gate_compact(answers, ctx_len, tau, expert_conf=None, conf_mode=CONF_VOTE, *
         _dptr(r["total_tokens"]), _dptr(r["max_seqlen"]), _dptr(r["workspace"]),
         r["workspace"].numel(), _stream(stream))
     _check("mosaic_gate_compact", st)
+    return r
+
+
+def gate_compact_tau(answers, ctx_len, tau_per_query, expert_conf=None, conf_mode=CONF_VOTE, *,
+                     out=None, stream=None):
+    """mosaic_gate_compact_tau: a threshold per question (fp32 [Q])."""
+    Q, E = answers.shape
+    dev = answers.device
+    o = out or {}
+    r = _compact_outputs(Q, dev, out)
+    r["mode"] = o.get("mode", torch.empty(Q, dtype=torch.int32, device=dev))
+    r["conf"] = o.get("conf", torch.empty(Q, dtype=torch.float32, device=dev))
+    r["bypass"] = o.get("bypass", torch.empty(Q, dtype=torch.uint8, device=dev))
+    st = load().mosaic_gate_compact_tau(
+        _dptr(answers, torch.int32, "answers"), _dptr(expert_conf, torch.float32, "expert_conf"),
+        _dptr(ctx_len, torch.int32, "ctx_len"), Q, E, _dptr(tau_per_query, torch.float32, "tau"),
+        conf_mode, _dptr(r["mode"]), None, None, _dptr(r["conf"]), _dptr(r["bypass"]),
+        _dptr(r["survivor_idx"]), _dptr(r["cu_seqlens"]), _dptr(r["n_survivors"]),
+        _dptr(r["total_tokens"]), _dptr(r["max_seqlen"]), _dptr(r["workspace"]),
+        r["workspace"].numel(), _stream(stream))
+    _check("mosaic_gate_compact_tau", st)
     return r
 
 
