@@ -132,6 +132,43 @@ def context_parts(cfg: Config, seed: int, Q: Optional[int] = None, E: Optional[i
     return prompt_tokens, prompt_off, trace_tokens, trace_off
 
 
+_A_N4 = 31
+# MMLU-Pro-shaped gate statistics (Table 1: 45.71 % of the questions are
+# 3:0 and 84.62 % are 3:0 or 2:1) and trace lengths that fall with agreement (mean
+# output 1 064 tokens for 3:0 against 2 696 for 1:1:1, 2.53 x, Spearman rho = -0.27).
+N4_BUCKET_RATES = (0.4571, 0.8462 - 0.4571, 1.0 - 0.8462)       # 3:0, 2:1, 1:1:1
+N4_MEAN_TOKENS = (1064.0, (1064.0 * 2696.0) ** 0.5, 2696.0)   # 2:1 is not printed: geometric mean
+N4_SIGMA, N4_CAP, N4_PROMPT = 1.15, 16384, 256
+
+
+def n4_inputs(seed: int, Q: int):
+    """k = 3 answers with the paper's bucket rates and, per expert trace, a lognormal length whose
+    mean depends on the question's bucket (sigma = 1.15 puts the Spearman correlation between
+    agreement and trace length, per (question, expert) sample, at the paper's -0.27).  Returns
+    (answers int32 [Q,3], ctx_len int32 [Q] = 256-token prompt + three traces, trace_len [Q,3])."""
+    g = rng(seed, 6, _A_N4)
+    b = g.choice(3, size=Q, p=np.asarray(N4_BUCKET_RATES) / sum(N4_BUCKET_RATES))
+    first = g.integers(0, 10, size=Q)
+    second = (first + g.integers(1, 10, size=Q)) % 10
+    third = (first + g.integers(1, 10, size=Q)) % 10
+    third = np.where(third == second, (third + 1) % 10, third)
+    third = np.where(third == first, (third + 1) % 10, third)
+    third = np.where(third == second, (third + 1) % 10, third)
+    odd = g.integers(0, 3, size=Q)  # which expert dissents in a 2:1 question
+    a = np.repeat(first[:, None], 3, axis=1)
+    two = b == 1
+    a[two, odd[two]] = second[two]
+    three = b == 2
+    a[three, 1] = second[three]
+    a[three, 2] = third[three]
+    mean = np.asarray(N4_MEAN_TOKENS)[b]
+    mu = np.log(mean) - N4_SIGMA ** 2 / 2
+    t_len = np.exp(mu[:, None] + N4_SIGMA * g.standard_normal((Q, 3)))
+    t_len = np.clip(np.rint(t_len), 1, N4_CAP).astype(np.int64)
+    ctx = (N4_PROMPT + t_len.sum(axis=1)).astype(np.int32)
+    return a.astype(np.int32), ctx, t_len
+
+
 @dataclass
 class GateInputs:
     answers: np.ndarray
