@@ -399,7 +399,7 @@ def bench_attn_kv(torch, mosaic, pk):
                          "unit": "TFLOP/s", "frac": fl / t / 1e12 / pk["bf16_tflops"], "traffic": None}}
 
 
-def bench_lse_merge(torch, mosaic, pk, T, Hq, D):
+def bench_lse_merge(torch, mosaic, pk, T, Hq, D, traffic=None):
     """mosaic_lse_merge on two partial results of the bench config's shape.
     Algorithmic bytes: two bf16 reads and one write per element of O, three fp32 LSE values per row."""
     dev = "cuda"
@@ -424,7 +424,7 @@ def bench_lse_merge(torch, mosaic, pk, T, Hq, D):
     return {"workload": "SURVEY 8(f) N2: LSE merge of two partials, T=%d, Hq/D=%d/%d" % (T, Hq, D),
             "us_per_call": t * 1e6,
             "roofline": {"bound": "hbm", "achieved": byts / t / 1e9, "peak": pk["hbm_gbs"],
-                         "unit": "GB/s", "frac": byts / t / 1e9 / pk["hbm_gbs"], "traffic": None,
+                         "unit": "GB/s", "frac": byts / t / 1e9 / pk["hbm_gbs"], "traffic": traffic,
                          "algorithmic_bytes": byts}}
 
 
@@ -636,7 +636,9 @@ def run_product(args):
     attn_kv_info = bench_attn_kv(torch, mosaic, pk)
     decode_info = bench_decode(torch, mosaic, pk)
     gated_info = bench_gated_stage(torch, mosaic, wl)
-    merge_info = bench_lse_merge(torch, mosaic, pk, T, cfg.Hq, cfg.D)
+    merge_info = bench_lse_merge(torch, mosaic, pk, T, cfg.Hq, cfg.D,
+                                 json.loads(tj0.read_text()).get("lse_merge_dram_bytes_per_launch")
+                                 if tj0.exists() else None)
     rope_info = bench_rope(torch, mosaic, pk, T, cfg.Hq, cfg.Hkv, cfg.D, rope_traffic)
     f, t, threads, desc = oracle_sample(cfg, 0, args.cpu_rows)
     attn_tflops = flops / (attn_ms * 1e-3) / 1e12
