@@ -41,20 +41,23 @@ __global__ void __launch_bounds__(kAsmThreads) assemble_kernel(const AssembleArg
     const int64_t L = p.cu_seqlens[j + 1] - t0;
     const int64_t i0 = (int64_t)blockIdx.y * kAsmChunk;
     if (i0 >= L) return;
-    const int nseg = p.E + 1;
+    const int nseg = p.E + 1;  // <= MOSAIC_MAX_EXPERTS + 1 = 33
     if (threadIdx.x < 32) {
-        // one lane per segment: the offset loads are one round trip, the prefix a warp scan
+        // one lane per segment (lane 0 also takes segment 32 when E = 32): the offset loads are one
+        // round trip, the prefix a full 32-lane warp scan
         const int g = threadIdx.x;
         const int64_t q = p.survivor_idx[j];
-        int64_t first = 0, len = 0;
-        if (g < nseg) {
-            const int64_t* off = g == 0 ? p.prompt_off + q : p.trace_off + q * p.E + (g - 1);
+        auto bounds = [&](int seg, int64_t& first, int64_t& len) {
+            const int64_t* off = seg == 0 ? p.prompt_off + q : p.trace_off + q * p.E + (seg - 1);
             first = off[0];
             len = off[1] - first;
-        }
+        };
+        int64_t first = 0, len = 0, first32 = 0, len32 = 0;
+        if (g < nseg) bounds(g, first, len);
+        if (g == 0 && nseg == 33) bounds(32, first32, len32);
         int64_t incl = len;
 #pragma unroll
-        for (int o = 1; o < 16; o <<= 1) {
+        for (int o = 1; o < 32; o <<= 1) {
             const int64_t y = __shfl_up_sync(0xffffffffu, incl, o);
             if (g >= o) incl += y;
         }
@@ -62,11 +65,17 @@ __global__ void __launch_bounds__(kAsmThreads) assemble_kernel(const AssembleArg
             cum[g] = incl - len;
             src[g] = (g == 0 ? p.prompt_tokens : p.trace_tokens) + first - (incl - len);
         }
-        if (g == nseg - 1) {
-            cum[nseg] = incl;
-            if (blockIdx.y == 0 && incl != L && p.n_mismatch) atomicAdd(p.n_mismatch, 1);
+        const int64_t sum32 = __shfl_sync(0xffffffffu, incl, 31);  // segments 0..31 (absent ones are 0)
+        if (g == 0) {
+            int64_t total = sum32;
+            if (nseg == 33) {
+                cum[32] = sum32;
+                src[32] = p.trace_tokens + first32 - sum32;
+                total += len32;
+            }
+            cum[nseg] = total;
+            if (blockIdx.y == 0 && total != L && p.n_mismatch) atomicAdd(p.n_mismatch, 1);
         }
-        // segments past E (none exist): never selected below because cum[k] is only read for k <= E
     }
     __syncthreads();
     const int64_t i1 = min(L, i0 + kAsmChunk);

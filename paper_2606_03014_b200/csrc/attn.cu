@@ -204,7 +204,7 @@ struct SmemLayout {
     static constexpr int kQ = 0;                    // Q_0, Q_1
     static constexpr int kKV = 2 * kTileBytes;      // ring of kSlots tiles
     static constexpr int kBars = kKV + kSlots * kTileBytes;
-    static constexpr int kStat = kBars + 512;       // (m, l) of every row of both tiles, for the epilogue
+    static constexpr int kStat = kBars + 512;       // (logsumexp, 1 / normaliser) of every row of both tiles, for the epilogue
     static constexpr int kUnits = kStat + 2 * BM * 8;  // ring of work-unit descriptors (32 bytes each)
     static constexpr int kTotal = kUnits + kUnitSlots * 32;
     static constexpr int kDynamic = kTotal;         // the base is 1024-byte aligned (checked)
@@ -221,7 +221,7 @@ enum Bar : uint32_t {
     kBarPFull = kBarSFull + 4,              // [2][2] P_t written over buffer b      (4 warps)
     kBarPvDone = kBarSFull + 8,             // [2]  a PV_t step complete             (commit)
     kBarODone = kBarSFull + 10,             // [2]  last PV_t of the item complete   (commit)
-    kBarStat = kBarSFull + 12,              // [2]  (m, l) of the tile's rows are in shared memory (4 warps)
+    kBarStat = kBarSFull + 12,              // [2]  (logsumexp, 1/normaliser) of the tile's rows are in shared memory (4 warps)
     kBarOFree = kBarSFull + 14,             // [2]  the epilogue has read O_t        (4 warps)
     kBarUnitFull = kBarSFull + 16,          // [kUnitSlots] the producer has published a work unit
     kBarUnitEmpty = kBarSFull + 16 + kUnitSlots,  // [kUnitSlots] every other role has read it (14 warps)
@@ -268,8 +268,10 @@ __device__ __forceinline__ Work make_work(const AttnParams& p, const int4 it, in
     k.lk = lk;
     k.row0 = it.z * BQ;
     // KV tiles of a q tile: up to the last key its last row sees (2c+1 and 2c+2 when off = 0)
-    const int last0 = min(min(k.row0 + BM, k.L) + k.off, lk);
-    const int last1 = min(min(k.row0 + BQ, k.L) + k.off, lk);
+    // (clamped at 0: a sequence without keys -- mosaic_agg_decode_attn makes those -- or, against
+    //  the contract, with fewer keys than q rows when causal, has tiles that visit nothing)
+    const int last0 = max(0, min(min(k.row0 + BM, k.L) + k.off, lk));
+    const int last1 = max(0, min(min(k.row0 + BQ, k.L) + k.off, lk));
     k.n0 = (last0 + BN - 1) / BN;
     k.n1 = (k.row0 + BM < k.L) ? (last1 + BN - 1) / BN : 0;
     k.n_kv = max(k.n0, k.n1);
@@ -407,10 +409,10 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                     ptx::mbar_wait(bar(kBarODone, t), ph[t]);  // ... and so is the last PV_t
                     ph[t] ^= 1;
                     ptx::tc_fence_after();
-                    const float2 ml = stat[t * BM + row];
+                    const float2 ml = stat[t * BM + row];  // (logsumexp, 1 / normaliser) of the row
                     const uint32_t tO = tmem + 256 + t * 128 + lane_off;
                     const int row_g = k.row0 + t * BM + row;
-                    const float inv_l = 1.f / ml.y;
+                    const float inv_l = ml.y;
                     __nv_bfloat16* orow = p.o + ((k.t0 + row_g) * p.Hq + k.h) * (int64_t)D;
 #pragma unroll 2
                     for (int c = 0; c < D / 16; ++c) {
@@ -445,8 +447,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                     ptx::tc_fence_before();
                     __syncwarp();
                     if (lane == 0) ptx::mbar_arrive(bar(kBarOFree, t));
-                    if (row_g < k.L)
-                        p.lse[(int64_t)k.h * p.T + k.t0 + row_g] = (ml.x + log2f(ml.y)) * kLn2;
+                    if (row_g < k.L) p.lse[(int64_t)k.h * p.T + k.t0 + row_g] = ml.x;
                 }
             }
         } else if (warp == kWarpProducer) {
@@ -518,7 +519,11 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                     }
                     __syncwarp();
                 };
-                load_q(0);
+                // A tile without KV tiles (n_t = 0) is skipped by its issuer, softmax group and
+                // epilogue: its Q must not be loaded either (nobody would release the buffer), and
+                // a unit without any KV tile takes no ring position at all.
+                if (k.n_kv == 0) continue;
+                if (k.n0) load_q(0);
                 load_kv(&tm_k, 0);
                 if (k.n1) load_q(1);
                 load_kv(&tm_v, 0);
@@ -669,7 +674,14 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         const int wq = warp & 3;                              // rows 32 wq .. 32 wq + 31 of the tile
         const float sc = p.scale_log2;
         uint32_t ph_s = 0, ph_f = 0;
-        float m_used = 0.f, l_run = 0.f;
+        // l_run: the row sum of the un-rounded P (what the logsumexp needs).  l_fix: the rounding
+        // residual bf16(p) - p of each step's LARGEST p.  O accumulates the bf16-rounded P, so its
+        // normaliser should be the sum of the rounded values; summing those would cost three more
+        // instructions per element pair, while correcting the step's top element is six per step
+        // and removes the whole error exactly where it matters: a nearly one-hot row (sharp
+        // softmax), where O = bf16(p_top) V / p_top was off by up to 2^-9 |V| -- with the running
+        // max moved lazily p_top is anything in [1, 2^8], not 1.
+        float m_used = 0.f, l_run = 0.f, l_fix = 0.f;
         int thr = 0;  // of the masked step in progress
 
         // One step: 64 scores of this row (buffer b) -> running max -> P (bf16, in place) -> row sum.
@@ -710,7 +722,8 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                     mx2 = fmaxf(mx2, s[c + 2]);
                     mx3 = fmaxf(mx3, s[c + 3]);
                 }
-                const float m_new = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * sc;
+                const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+                const float m_new = mx * sc;
                 if (first) {
                     m_used = m_new;
                 } else {
@@ -726,6 +739,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                         const float alpha = need ? ex2_approx(m_used - m_new) : 1.f;
                         if (need) m_used = m_new;
                         l_run *= alpha;
+                        l_fix *= alpha;
 #pragma unroll 1  // rare: keep it small (instruction cache)
                         for (int c = 0; c < D / 16; ++c) {
                             uint32_t r[16];
@@ -742,6 +756,13 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                 // Two elements at a time (packed fp32 FMA / ADD).  Of every four pairs, kPolyPairs
                 // are exponentiated on the FMA pipe (exp2_poly2) and the rest on the MUFU unit
                 // (16 results per clock per SM; DESIGN.md says why kPolyPairs is 0).
+#ifndef MOSAIC_NO_TOP_FIX
+                {   // the step's top element, by the same FMA and ex2 as in the loop below
+                    float e_top = ex2_approx(fmaf(mx, sc, -m_used));
+                    if constexpr (kMask == 1) e_top = mx == -INFINITY ? 0.f : e_top;
+                    l_fix += __bfloat162float(__float2bfloat16_rn(e_top)) - e_top;
+                }
+#endif
                 float2 la = make_float2(0.f, 0.f), lb = make_float2(0.f, 0.f);
                 const float2 sc2 = make_float2(sc, sc), nm2 = make_float2(-m_used, -m_used);
 #pragma unroll
@@ -790,6 +811,7 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             if (n_t == 0) continue;  // this tile has no rows in this block
             m_used = 0.f;
             l_run = 0.f;
+            l_fix = 0.f;
             // Row r of the sequence sees keys j <= r + off.  Steps whose 64 keys every row of the tile
             // sees run unmasked, in pairs (one copy per buffer); from the first step that some row of
             // the tile does not see in full, a warp's 32 rows x 64 keys are either masked altogether
@@ -813,12 +835,13 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                     step(M1{}, b, u == 0);
                 ph_s ^= (uint32_t)b;
             }
-            // ---- hand the row's (m, l) to the epilogue warps and go on to the next item -----------
+            // ---- hand the row's (logsumexp, 1 / normaliser) to the epilogue warps and go on to the next item -----------
             // (first make sure the epilogue has read the previous item's pair -- it releases O_t
             //  after that; an item of a single KV tile gets here without PV_t(0) having waited)
             ptx::mbar_wait(bar(kBarOFree, t), ph_f ^ 1);
             ph_f ^= 1;
-            reinterpret_cast<float2*>(smem + SL::kStat)[t * BM + row] = make_float2(m_used, l_run);
+            reinterpret_cast<float2*>(smem + SL::kStat)[t * BM + row] =
+                make_float2((m_used + log2f(l_run)) * kLn2, 1.f / (l_run + l_fix));
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(bar(kBarStat, t));
         }

@@ -212,10 +212,16 @@ extern "C" mosaic_status_t mosaic_stage_host(
         MOSAIC_CUDA_TRY(cudaMemcpyAsync(at_w(a.v, t0 * kv_row), at(v_h, t0 * kv_row), rows * kv_row, H2D, pp.in));
         MOSAIC_CUDA_TRY(cudaEventRecord(pp.ev_in[c], pp.in));
         MOSAIC_CUDA_TRY(cudaStreamWaitEvent(s, pp.ev_in[c], 0));
-        // the sequences s0 .. s1-1 of the same packed buffers: cu_seqlens holds absolute offsets
-        st = mosaic_agg_prefill_attn(a.q, a.k, a.v, a.cu_seqlens + s0, (int32_t)(s1 - s0), T,
-                                     sc.max_len, Hq, Hkv, D, softmax_scale, a.o, a.lse, a.attn_ws,
-                                     a.attn_ws_bytes, s);
+        // The sequences s0 .. s1-1 of the same packed buffers: cu_seqlens holds absolute offsets.
+        // K and V are declared only as far as this chunk's last token (total_k_tokens = t1): the
+        // last 128-row K / V box of the chunk reaches past it into rows whose copy (chunk c + 1)
+        // may still be in flight -- those rows are masked, but a masked P = 0 times a stale NaN
+        // pattern in V would still be NaN -- and rows past the tensor map's extent are zero-filled
+        // by the TMA unit instead of being read.
+        st = mosaic_agg_prefill_attn_kv(a.q, a.k, a.v, a.cu_seqlens + s0, a.cu_seqlens + s0,
+                                        (int32_t)(s1 - s0), T, t1, sc.max_len, Hq, Hkv, D,
+                                        softmax_scale, /*causal=*/1, a.o, a.lse, a.attn_ws,
+                                        a.attn_ws_bytes, s);
         if (st != MOSAIC_OK) {
             cudaStreamSynchronize(pp.in);
             cudaStreamSynchronize(s);

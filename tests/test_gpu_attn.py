@@ -62,14 +62,37 @@ def test_half_tile_edges_full():
     assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
 
 
-def test_rescale_path_many_steps():
+def _error_split(lengths, Hq, Hkv, D, seed, k_scale, v_scale):
+    """(total, rounding, arithmetic) max abs errors of O: |O_gpu - O_oracle|, the share the bf16
+    output format alone costs, |bf16_rn(O_oracle) - O_oracle|, and |O_gpu - bf16_rn(O_oracle)|."""
+    cu = _cu(lengths)
+    T = int(cu[-1])
+    q = P.randn_bf16((T, Hq, D), seed)
+    k = P.randn_bf16((T, Hkv, D), seed + 1, k_scale)
+    v = P.randn_bf16((T, Hkv, D), seed + 2, v_scale)
+    scale = 1.0 / np.sqrt(D)
+    o, lse = P.run_attn(q, k, v, cu, scale)
+    O_ref, lse_ref = oracle.attn_full(P.bf16_bits(q), P.bf16_bits(k), P.bf16_bits(v), cu, scale)
+    got = o.float().cpu().numpy().astype(np.float64)
+    rn = torch.from_numpy(O_ref).to(torch.bfloat16).double().numpy()
+    el = float(np.abs(lse.cpu().numpy() - lse_ref).max())
+    return (float(np.abs(got - O_ref).max()), float(np.abs(rn - O_ref).max()),
+            float(np.abs(got - rn).max()), float(np.abs(O_ref).max()), el)
+
+
+@pytest.mark.parametrize("v_scale", [1.0, 0.25])
+def test_rescale_path_many_steps(v_scale):
     """K x 64: the running max jumps by far more than the lazy-rescale threshold (2^8) again and
     again over ~40 steps, so O is rescaled in tensor memory behind the PV commit barrier.  The rows
-    are nearly one-hot, so O is a single V row: V x 0.25 keeps |O| <= ~1.2, where the bf16 rounding of
-    the output (2^-9 |O|) stays inside the absolute tolerance that DESIGN.md derives for |O| ~ 1."""
+    are nearly one-hot, so O is close to a single V row.  Run at V ~ N(0,1) (max |O| ~ 4.5, where one
+    bf16 rounding of the OUTPUT alone is up to 2^-7 = 7.8e-3 in [2, 4) and 1.6e-2 in [4, 8)) and at
+    V x 0.25; the split of the error into output rounding and arithmetic is printed and the total
+    is held to north_star's tolerance in both."""
     for D in (128, 64):
-        eo, el = _full_case([1300, 2600, 70], 2, 1, D, seed=23, k_scale=64.0, v_scale=0.25)
-        assert eo <= P.O_TOL and el <= P.LSE_TOL, (D, eo, el)
+        tot, rnd, arith, omax, el = _error_split([1300, 2600, 70], 2, 1, D, 23, 64.0, v_scale)
+        print(f"rescale path D={D} V x {v_scale}: max|O|={omax:.2f} total={tot:.3e} "
+              f"bf16-rounding-alone={rnd:.3e} gpu-vs-rounded-oracle={arith:.3e} dLSE={el:.2e}")
+        assert tot <= P.O_TOL and el <= P.LSE_TOL, (D, v_scale, tot, rnd, arith, el)
 
 
 def test_sharp_softmax_and_scales():
@@ -223,13 +246,20 @@ def test_stage_host_chunked_matches_oracle():
     assert T > 8 * 16384
     q, k, v = wl.qkv(cfg, 0, T)
     scale = wl.softmax_scale(cfg)
-    r = mosaic.stage_host(torch.from_numpy(gi.answers), None, torch.from_numpy(gi.ctx_len), gi.tau,
-                          0, q, k, v, scale)
+    # The device arena starts as 0xFF bytes (bf16 NaN everywhere): chunk c's attention runs while
+    # chunk c + 1 is still being copied, and the last K / V tile of a chunk reaches past its end --
+    # a result that depends on the stale rows there shows up as NaN (check_attn_rows asserts finite).
+    arena = torch.full((mosaic.stage_host_arena_bytes(cfg.Q, cfg.E, T, cfg.Hq, cfg.Hkv, cfg.D),),
+                       0xFF, dtype=torch.uint8, device="cuda")
+    r = mosaic.stage_host(torch.from_numpy(gi.answers).pin_memory(), None,
+                          torch.from_numpy(gi.ctx_len).pin_memory(), gi.tau, 0, q.pin_memory(),
+                          k.pin_memory(), v.pin_memory(), scale, arena=arena)
     S = int(r["n_survivors"])
     assert S == want["n_survivors"] and int(r["total_tokens"]) == T
     assert np.array_equal(r["bypass"].numpy(), want["bypass"])
     assert np.array_equal(r["survivor_idx"][:S].numpy(), want["survivor_idx"])
     assert np.array_equal(r["cu_seqlens"][:S + 1].numpy(), cu)
+    assert bool(torch.isfinite(r["o"][:T].float()).all()) and bool(torch.isfinite(r["lse"][:cfg.Hq * T]).all())
     rs, rh, rp = wl.sample_rows(cu, cfg.Hq, cfg.Hkv, 0, cfg.config_id, n_random=256)
     o = r["o"][:T]
     lse = r["lse"][:cfg.Hq * T].view(cfg.Hq, T)

@@ -103,9 +103,12 @@ def test_split_kv_prefill_merged_on_the_gpu():
                                      cu_n, 1, n, scale)
     o, lse = mosaic.lse_merge(o1, l1, o2, l2)
     torch.cuda.synchronize()
-    # two bf16 roundings of O (the partials, then the merge) instead of one
-    assert np.abs(o.float().cpu().numpy() - O_ref[a:]).max() <= 1.5 * P.O_TOL
-    assert np.abs(lse.cpu().numpy() - lse_ref[:, a:]).max() <= P.LSE_TOL
+    # A merged result carries two bf16 roundings of O (the partials, then the merge) instead of
+    # one; it is held to north_star's plain tolerance all the same (measured on a B200: 1.6e-3).
+    eo = float(np.abs(o.float().cpu().numpy() - O_ref[a:]).max())
+    el = float(np.abs(lse.cpu().numpy() - lse_ref[:, a:]).max())
+    print(f"split-KV merge: max|dO|={eo:.3e} max|dLSE|={el:.2e} (tolerances {P.O_TOL:.0e} / {P.LSE_TOL:.0e})")
+    assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
 
 
 def test_merge_against_the_oracle_and_empty_partials():

@@ -106,3 +106,20 @@ def test_too_small_workspace_is_an_error():
     with pytest.raises(mosaic.MosaicError) as e:
         mosaic.compact(by, cl, out=dict(workspace=torch.empty(64, dtype=torch.uint8, device="cuda")))
     assert e.value.status == mosaic.ERR_WORKSPACE_TOO_SMALL
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_n4_paper_shaped_workload_bit_exact(seed):
+    """the paper-shaped inputs bench.py's gated-stage leg runs (k = 3, MMLU-Pro bucket
+    rates, trace lengths falling with agreement) through the gate and the
+    compaction at the paper's two operating points (tau = 2/3 and 1) against the oracle."""
+    for Q in (768, 50000):
+        a, ctx, _ = wl.n4_inputs(seed, Q)
+        for tau in (2.0 / 3.0, 1.0):
+            gi = wl.GateInputs(a, None, ctx, tau, 3)
+            want = P.oracle_gate_compact(gi, 0)
+            sep, fused = P.gpu_gate_compact_all(gi, 0)
+            P.assert_gate_equal(sep, want)
+            P.assert_gate_equal(fused, want)
+        assert 0.80 < 1.0 - P.oracle_gate_compact(wl.GateInputs(a, None, ctx, 2.0 / 3.0, 3), 0)[
+            "n_survivors"] / Q < 0.89   # Table 1: 84.62 % skipped at tau = 2/3
