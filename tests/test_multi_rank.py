@@ -52,3 +52,32 @@ def test_two_ranks_whole_job_aggregate():
 def test_single_rank_is_identity():
     import bench
     assert bench.whole_job(0.5, 7.0, 1) == (0.5, 7.0)
+
+
+def _spawned(out):
+    """What bench.py --gpus N runs in every rank it starts itself, on gloo: the environment that
+    spawn_ranks sets up is the one torchrun would have set."""
+    rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+    assert int(os.environ["LOCAL_RANK"]) == rank and os.environ["MASTER_ADDR"] == "127.0.0.1"
+    dist.init_process_group("gloo")
+    import bench
+    out[rank] = bench.whole_job(1.0 + rank, 10.0 * (rank + 1), world)
+    dist.destroy_process_group()
+
+
+def test_bench_spawns_its_own_ranks():
+    """`bench.py --gpus N` without a launcher starts N ranks itself (bench.spawn_ranks)."""
+    import bench
+    with mp.Manager() as m:
+        out = m.dict()
+        bench.spawn_ranks(2, _spawned, (out,))
+        assert out[0] == out[1] == (2.0, 30.0)
+
+
+def test_gpus_flag_must_match_the_world_size():
+    """A rank whose --gpus differs from WORLD_SIZE refuses to run (no N-labelled single-GPU line)."""
+    import subprocess
+    env = dict(os.environ, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0")
+    r = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--gpus", "2", "--steps", "1"],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode != 0 and "WORLD_SIZE" in (r.stderr + r.stdout)
