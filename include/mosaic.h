@@ -16,8 +16,11 @@
  * Conventions (all entry points)
  *   - Pointers marked [dev] are CUDA device pointers, 16-byte aligned, owned by the caller.
  *     Pointers marked [host] are ordinary host pointers.  The library allocates no device
- *     memory and keeps no state between calls; scratch comes from caller workspaces sized by
- *     the *_workspace_bytes helpers.
+ *     memory; scratch comes from caller workspaces sized by the *_workspace_bytes helpers, whose
+ *     contents may be arbitrary on entry.  No call depends on an earlier one: what the library
+ *     keeps per process is caches only (kernel attributes, occupancy figures, the tensor-map
+ *     encoder entry point) and, for mosaic_stage_host alone, two copy streams and their events,
+ *     created on first use and kept until the process exits.
  *   - cuda_stream is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls
  *     marked "async" only enqueue work on that stream and never synchronise.
  *   - Errors are return codes; nothing is thrown or printed.  Host-visible arguments are
@@ -48,7 +51,17 @@ typedef enum {
  * confidence estimator"). */
 enum {
     MOSAIC_CONF_VOTE = 0,     /* C_vote = plurality fraction, the paper's instantiation */
-    MOSAIC_CONF_WEIGHTED = 1  /* extension (reading G-10): weight share of the modal answer */
+    MOSAIC_CONF_WEIGHTED = 1, /* extension (reading G-10): weight share of the modal answer */
+    MOSAIC_CONF_WEIGHTED_ARGMAX = 2 /* extension (reading N3-3): the answer is the label with the
+                                       LARGEST weight sum (ties -> smallest label), C its share */
+};
+
+/* What a failed Extract (Alg. 1 line 1) does to the vote (reading N3-2): an
+ * expert whose label equals the caller's sentinel abstains and is left out of every tally. */
+enum {
+    MOSAIC_ABSTAIN_NONE = 0,     /* no sentinel: every label is an answer (reading G-6)               */
+    MOSAIC_ABSTAIN_KEEP_K = 1,   /* C still divides by the k experts recruited (P:L182 literally)     */
+    MOSAIC_ABSTAIN_SHRINK_K = 2  /* C divides by the experts that answered                            */
 };
 
 #define MOSAIC_MAX_EXPERTS 32
@@ -58,8 +71,8 @@ enum {
  *
  *   answers     [dev] int32 [Q, E] row-major (question-major): a_i = Extract(E_i(q)).
  *                     Any int32 is a label; only equality matters.
- *   expert_conf [dev] fp32 [Q, E] per-response weights w; required iff conf_mode == WEIGHTED,
- *                     else may be NULL.
+ *   expert_conf [dev] fp32 [Q, E] per-response weights w; required iff conf_mode != VOTE, else
+ *                     may be NULL.
  *   Q, E              0 <= Q < 2^31, 1 <= E <= MOSAIC_MAX_EXPERTS (the paper's k; k = 3 at P:L331).
  *   tau               threshold, compared in fp32 (reading G-4); NaN -> INVALID_ARG.
  *   mode_out    [dev] int32 [Q]  majority({a_i}); ties -> smallest label (reading G-2). May be NULL.
@@ -68,6 +81,10 @@ enum {
  *   conf_out    [dev] fp32  [Q]  the C(q) the gate compared: agree (VOTE) or
  *                                fl32(sum_{i: a_i = mode} w_i / sum_i w_i) with binary64 sums in
  *                                expert order, agree when sum_i w_i <= 0 (WEIGHTED).  May be NULL.
+ *                                WEIGHTED_ARGMAX: the same share with mode = the label whose
+ *                                weight sum is largest (ties -> smallest label); count_out is
+ *                                then that label's votes and agree_out = count / E; when
+ *                                sum_i w_i <= 0 the call falls back to VOTE for the question.
  *   bypass_out  [dev] uint8 [Q]  1 iff C(q) >= tau (aggregator skipped, answer = mode). Required.
  *
  * Q == 0 is a successful no-op.
@@ -126,8 +143,9 @@ mosaic_status_t mosaic_gate_compact(const int32_t* answers, const float* expert_
  *   q            [dev] bf16 [T, Hq, D]   packed, D fastest, no padding between sequences.
  *   k, v         [dev] bf16 [T, Hkv, D]
  *   cu_seqlens   [dev] int64 [n_seqs+1]  cu[0] = 0, non-decreasing, cu[n_seqs] = total_tokens.
- *   n_seqs, total_tokens, max_seqlen     HOST values; max_seqlen >= every sequence length.
- *                                        0 <= total_tokens < 2^31.
+ *   n_seqs, total_tokens, max_seqlen     HOST values; max_seqlen >= every sequence length (only
+ *                                        its sign is checked today: the work list is built on
+ *                                        the device from cu_seqlens).  0 <= total_tokens < 2^31.
  *   Hq, Hkv, D                           Hq % Hkv == 0; D in {64, 128} (else UNSUPPORTED).
  *   softmax_scale                        finite fp32 (the configs use 1/sqrt(D)).
  *   o            [dev] bf16 [T, Hq, D]   fp32 accumulator rounded to nearest-even.
@@ -164,6 +182,44 @@ mosaic_status_t mosaic_gate_compact_tau(const int32_t* answers, const float* exp
                                         size_t workspace_bytes, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * mosaic_gate_compact_ext -- SURVEY.md section 8(f) N3: mosaic_gate_compact with every optional
+ * estimator setting in one call.  P:L188: the gate "is agnostic to the choice of confidence
+ * estimator"; `Extract` may fail; a static tau is a stated limitation.
+ *   tau_per_query  [dev] fp32 [Q] or NULL (then `tau` for every question), as mosaic_gate_compact_tau.
+ *   conf_mode      MOSAIC_CONF_VOTE / _WEIGHTED / _WEIGHTED_ARGMAX.
+ *   abstain_policy MOSAIC_ABSTAIN_*; abstain_label is the sentinel `Extract` returns on failure.
+ *                  An abstaining expert is not counted for any label, cannot be the mode, and adds
+ *                  no weight to a label; with KEEP_K the denominators stay E (votes) and
+ *                  sum over ALL experts of w (weights), with SHRINK_K they run over the experts
+ *                  that answered.  If every expert abstains: mode = abstain_label, count = 0,
+ *                  agree = conf = 0 (the question bypasses only when tau <= 0).
+ * Every other argument, the outputs and the errors as mosaic_gate_compact.
+ * ------------------------------------------------------------------------------------------- */
+mosaic_status_t mosaic_gate_compact_ext(const int32_t* answers, const float* expert_conf,
+                                        const int32_t* ctx_len, int64_t Q, int32_t E, float tau,
+                                        const float* tau_per_query, int32_t conf_mode,
+                                        int32_t abstain_policy, int32_t abstain_label,
+                                        int32_t* mode_out, int32_t* count_out, float* agree_out,
+                                        float* conf_out, uint8_t* bypass_out, int32_t* survivor_idx,
+                                        int64_t* cu_seqlens, int32_t* n_survivors,
+                                        int64_t* total_tokens, int32_t* max_seqlen, void* workspace,
+                                        size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * mosaic_conf_compact -- SURVEY.md section 8(f) N3: Alg. 1 lines 4-6 on a confidence the CALLER
+ * computed ("response-level uncertainty, or context-aware features" may replace C_vote):
+ *     bypass[q] = conf[q] >= tau (or tau_per_query[q]), fp32 compare, NaN never bypasses;
+ * then the compaction of mosaic_compact, in the same launch.
+ *   conf [dev] fp32 [Q]; tau_per_query [dev] fp32 [Q] or NULL; bypass_out [dev] uint8 [Q] or NULL;
+ *   the remaining arguments as mosaic_compact.  NaN `tau` without tau_per_query -> INVALID_ARG.
+ * ------------------------------------------------------------------------------------------- */
+mosaic_status_t mosaic_conf_compact(const float* conf, const int32_t* ctx_len, int64_t Q, float tau,
+                                    const float* tau_per_query, uint8_t* bypass_out,
+                                    int32_t* survivor_idx, int64_t* cu_seqlens, int32_t* n_survivors,
+                                    int64_t* total_tokens, int32_t* max_seqlen, void* workspace,
+                                    size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * mosaic_agg_prefill_attn_kv -- SURVEY.md section 8(f) N2 (a "next" row): the same attention with
  * the q rows and the keys of a sequence packed separately, for prefix-cached prompts and chunked
  * prefill of the aggregator's long contexts (32 k-class windows): sequence s has Lq q rows
@@ -179,7 +235,9 @@ mosaic_status_t mosaic_gate_compact_tau(const int32_t* answers, const float* exp
  *   causal: 1 as above; 0: every q row sees ALL Lk keys of its sequence (the partial result of a
  *   block of earlier keys in a split-KV prefill; Lk >= 1 wherever Lq >= 1) -- see mosaic_lse_merge.
  * Everything else (alignment, D, errors, asynchrony) as mosaic_agg_prefill_attn.  Lk < Lq with
- * causal = 1 is not checked and not supported.
+ * causal = 1 is outside the contract and cannot be checked on the host (the lengths are device
+ * data): the kernel then visits no key tile for the q tiles that see none and finishes, but the
+ * O / LSE rows of such a sequence are unspecified.
  * ------------------------------------------------------------------------------------------- */
 mosaic_status_t mosaic_agg_prefill_attn_kv(const void* q, const void* k, const void* v,
                                            const int64_t* cu_seqlens_q,

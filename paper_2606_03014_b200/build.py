@@ -14,7 +14,9 @@ CSRC = PKG / "csrc"
 INCLUDE = ROOT / "include"
 LIB = PKG / "libmosaic.so"
 OBJ_DIR = PKG / "build"
-SOURCES = ["core.cu", "gate.cu", "attn.cu", "stage.cu", "assemble.cu", "rope.cu", "merge.cu", "decode.cu"]
+SOURCES = ["core.cu", "gate.cu", "compact.cu", "compact_inst_c0a0.cu", "compact_inst_c0a1.cu",
+           "compact_inst_c1a0.cu", "compact_inst_c1a1.cu", "compact_inst_c2a0.cu",
+           "compact_inst_c2a1.cu", "attn.cu", "stage.cu", "assemble.cu", "rope.cu", "merge.cu", "decode.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC",
               f"-I{INCLUDE}", f"-I{CSRC}"]
@@ -35,7 +37,8 @@ def _stale(target: Path, deps) -> bool:
 
 
 def build_library(force: bool = False, verbose: bool = False) -> Path:
-    headers = list(CSRC.glob("*.cuh")) + list(INCLUDE.glob("*.h")) + [Path(__file__)]
+    headers = (list(CSRC.glob("*.cuh")) + list(CSRC.glob("*.inc")) + list(INCLUDE.glob("*.h"))
+               + [Path(__file__)])
     OBJ_DIR.mkdir(exist_ok=True)
     nvcc = _nvcc()
 

@@ -1,0 +1,5 @@
+// Instantiation unit of compact_inst.inc: confidence estimator 1, abstention off.
+#define MOSAIC_INST_CONF 1
+#define MOSAIC_INST_ABSTAIN 0
+#define MOSAIC_INST_NAME dispatch_gate_c1a0
+#include "compact_inst.inc"

@@ -15,7 +15,8 @@ _PKG = Path(__file__).resolve().parent
 LIB_PATH = _PKG / "libmosaic.so"
 
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE_TOO_SMALL, ERR_CUDA = range(5)
-CONF_VOTE, CONF_WEIGHTED = 0, 1
+CONF_VOTE, CONF_WEIGHTED, CONF_WEIGHTED_ARGMAX = 0, 1, 2
+ABSTAIN_NONE, ABSTAIN_KEEP_K, ABSTAIN_SHRINK_K = 0, 1, 2
 
 _vp, _i32, _i64, _f32, _sz = (ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_float,
                               ctypes.c_size_t)
@@ -29,6 +30,11 @@ SIGNATURES = {
                                            _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     "mosaic_gate_compact_tau": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _vp, _i32, _vp, _vp, _vp,
                                                _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "mosaic_gate_compact_ext": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _f32, _vp, _i32, _i32, _i32,
+                                               _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp,
+                                               _sz, _vp]),
+    "mosaic_conf_compact": (ctypes.c_int, [_vp, _vp, _i64, _f32, _vp, _vp, _vp, _vp, _vp, _vp, _vp,
+                                           _vp, _sz, _vp]),
     "mosaic_agg_prefill_attn_workspace_bytes": (_sz, [_i32, _i64, _i32, _i32, _i32]),
     "mosaic_agg_prefill_attn": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i64, _i32, _i32, _i32,
                                                _i32, _f32, _vp, _vp, _vp, _sz, _vp]),
@@ -198,6 +204,49 @@ def gate_compact_tau(answers, ctx_len, tau_per_query, expert_conf=None, conf_mod
         _dptr(r["total_tokens"]), _dptr(r["max_seqlen"]), _dptr(r["workspace"]),
         r["workspace"].numel(), _stream(stream))
     _check("mosaic_gate_compact_tau", st)
+    return r
+
+
+def gate_compact_ext(answers, ctx_len, tau, expert_conf=None, conf_mode=CONF_VOTE, *,
+                     tau_per_query=None, abstain_policy=ABSTAIN_NONE, abstain_label=-1,
+                     want_count=True, want_agree=True, out=None, stream=None):
+    """mosaic_gate_compact_ext: per-question thresholds, the weighted-argmax
+    estimator and the abstention sentinel of a failed Extract, all optional, in one launch."""
+    Q, E = answers.shape
+    dev = answers.device
+    o = out or {}
+    r = _compact_outputs(Q, dev, out)
+    r["mode"] = o.get("mode", torch.empty(Q, dtype=torch.int32, device=dev))
+    r["count"] = o.get("count", torch.empty(Q, dtype=torch.int32, device=dev) if want_count else None)
+    r["agree"] = o.get("agree", torch.empty(Q, dtype=torch.float32, device=dev) if want_agree else None)
+    r["conf"] = o.get("conf", torch.empty(Q, dtype=torch.float32, device=dev))
+    r["bypass"] = o.get("bypass", torch.empty(Q, dtype=torch.uint8, device=dev))
+    st = load().mosaic_gate_compact_ext(
+        _dptr(answers, torch.int32, "answers"), _dptr(expert_conf, torch.float32, "expert_conf"),
+        _dptr(ctx_len, torch.int32, "ctx_len"), Q, E, float(tau),
+        _dptr(tau_per_query, torch.float32, "tau_per_query"), conf_mode, int(abstain_policy),
+        int(abstain_label), _dptr(r["mode"]), _dptr(r["count"]), _dptr(r["agree"]), _dptr(r["conf"]),
+        _dptr(r["bypass"]), _dptr(r["survivor_idx"]), _dptr(r["cu_seqlens"]), _dptr(r["n_survivors"]),
+        _dptr(r["total_tokens"]), _dptr(r["max_seqlen"]), _dptr(r["workspace"]),
+        r["workspace"].numel(), _stream(stream))
+    _check("mosaic_gate_compact_ext", st)
+    return r
+
+
+def conf_compact(conf, ctx_len, tau, *, tau_per_query=None, out=None, stream=None):
+    """mosaic_conf_compact: threshold + compaction on a confidence C(q) the
+    caller computed (fp32 [Q])."""
+    Q = conf.shape[0]
+    o = out or {}
+    r = _compact_outputs(Q, conf.device, out)
+    r["bypass"] = o.get("bypass", torch.empty(Q, dtype=torch.uint8, device=conf.device))
+    st = load().mosaic_conf_compact(
+        _dptr(conf, torch.float32, "conf"), _dptr(ctx_len, torch.int32, "ctx_len"), Q, float(tau),
+        _dptr(tau_per_query, torch.float32, "tau_per_query"), _dptr(r["bypass"]),
+        _dptr(r["survivor_idx"]), _dptr(r["cu_seqlens"]), _dptr(r["n_survivors"]),
+        _dptr(r["total_tokens"]), _dptr(r["max_seqlen"]), _dptr(r["workspace"]),
+        r["workspace"].numel(), _stream(stream))
+    _check("mosaic_conf_compact", st)
     return r
 
 
