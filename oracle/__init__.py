@@ -45,6 +45,9 @@ def _load():
         lib.oracle_gate.argtypes = [p, p, ctypes.c_int64, ctypes.c_int32, ctypes.c_float,
                                     ctypes.c_int32, p, p, p, p, p]
         lib.oracle_gate.restype = None
+        lib.oracle_gate_ext.argtypes = [p, p, ctypes.c_int64, ctypes.c_int32, ctypes.c_float, p,
+                                        ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, p, p, p, p, p]
+        lib.oracle_gate_ext.restype = None
         lib.oracle_compact.argtypes = [p, p, ctypes.c_int64, p, p, p, p]
         lib.oracle_compact.restype = ctypes.c_int64
         lib.oracle_attn_rows.argtypes = [p, p, p, p, ctypes.c_int64, p, p, p, ctypes.c_int32,
@@ -106,6 +109,44 @@ def gate_tau_per_query(answers, tau_q, expert_conf=None, conf_mode: int = 0):
     assert tau_q.shape == out["conf"].shape
     out["bypass"] = (out["conf"] >= tau_q).astype(np.uint8)
     return out
+
+
+def gate_ext(answers, tau, expert_conf=None, conf_mode: int = 0, tau_q=None,
+             abstain_policy: int = 0, abstain_label: int = -1):
+    """the gate with the optional estimator settings (oracle_gate_ext in the C
+    source states them): conf_mode 2 = the answer is the label with the largest weight sum
+    (reading N3-3); tau_q = a threshold per question (N3-1); abstain_policy 1 / 2 = an expert
+    whose label is abstain_label did not answer, C still divides by E (1) or by the experts that
+    answered (2) (N3-2).  Returns dict(mode, count, agree, conf, bypass)."""
+    answers = _c(answers, np.int32)
+    Q, E = answers.shape
+    if conf_mode not in (0, 1, 2) or abstain_policy not in (0, 1, 2):
+        raise ValueError("conf_mode / abstain_policy")
+    w = None
+    if conf_mode != 0:
+        w = _c(expert_conf, np.float32)
+        assert w.shape == (Q, E)
+    tq = None
+    if tau_q is not None:
+        tq = _c(tau_q, np.float32)
+        assert tq.shape == (Q,)
+    out = dict(mode=np.empty(Q, np.int32), count=np.empty(Q, np.int32),
+               agree=np.empty(Q, np.float32), conf=np.empty(Q, np.float32),
+               bypass=np.empty(Q, np.uint8))
+    _load().oracle_gate_ext(_ptr(answers), _ptr(w), Q, E, ctypes.c_float(np.float32(tau)), _ptr(tq),
+                            conf_mode, abstain_policy, int(abstain_label), _ptr(out["mode"]),
+                            _ptr(out["count"]), _ptr(out["agree"]), _ptr(out["conf"]),
+                            _ptr(out["bypass"]))
+    return out
+
+
+def conf_gate(conf, tau, tau_q=None):
+    """Alg. 1 line 4 on a confidence C(q) the caller computed:
+    bypass[q] = conf[q] >= tau (or tau_q[q]) in fp32; a NaN on either side never bypasses."""
+    c = _c(conf, np.float32)
+    t = np.float32(tau) if tau_q is None else _c(tau_q, np.float32)
+    with np.errstate(invalid="ignore"):
+        return (c >= t).astype(np.uint8)
 
 
 def compact(bypass, ctx_len):

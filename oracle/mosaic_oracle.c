@@ -249,3 +249,89 @@ int oracle_num_threads(void)
 #endif
     return n;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * the gate with the other confidence estimators P:L188 invites ("agnostic to
+ * the choice of confidence estimator"), a threshold per question (P:L251 names the static
+ * threshold as a limitation) and a failed Extract (Alg. 1 line 1).  Readings
+ * (DESIGN.md section 2): N3-1 tau per question; N3-2 abstention; N3-3 weighted argmax.
+ *
+ *   for each question q with answers a_1..a_E and (conf_mode 1, 2) weights w_1..w_E:
+ *     expert i ABSTAINS iff abstain_policy != 0 and a_i == abstain_label; an abstaining expert
+ *       is counted for no label and adds its weight to no label
+ *     n(x) = |{ i answering : a_i = x }|,  s(x) = sum_{i answering, a_i = x} w_i  (binary64,
+ *       increasing i)
+ *     k  = E                          (policy 0, 1: P:L182 divides by the k experts recruited)
+ *        = |{ i answering }|          (policy 2)
+ *     St = sum of w_i over all i (policy 0, 1) or over the answering i (policy 2), increasing i
+ *     mode:  conf_mode 0, 1, or St <= 0: the x with the largest n(x), ties -> smallest x
+ *            conf_mode 2 and St > 0    : the x with the largest s(x), ties -> smallest x
+ *            nobody answers            : abstain_label, with count 0
+ *     count = n(mode);  agree = fl32(count) / fl32(k)  (0 when k == 0)
+ *     conf  = agree                        (conf_mode 0, or St <= 0)
+ *           = fl32( s(mode) / St )         (conf_mode 1, 2)
+ *     bypass = conf >= (tau_q ? tau_q[q] : tau), fp32 comparison, false for a NaN threshold
+ *
+ * With policy 0, conf_mode 0 / 1 and tau_q == NULL this is oracle_gate.
+ * ---------------------------------------------------------------------------------------- */
+void oracle_gate_ext(const int32_t *answers, const float *expert_conf, int64_t Q, int32_t E,
+                     float tau, const float *tau_q, int32_t conf_mode, int32_t abstain_policy,
+                     int32_t abstain_label, int32_t *mode_out, int32_t *count_out,
+                     float *agree_out, float *conf_out, uint8_t *bypass_out)
+{
+    for (int64_t q = 0; q < Q; ++q) {
+        const int32_t *a = answers + q * (int64_t)E;
+        const float *w = conf_mode ? expert_conf + q * (int64_t)E : NULL;
+        int32_t answering = 0;
+        double st = 0.0;
+        for (int32_t i = 0; i < E; ++i) {
+            const int abst = abstain_policy != 0 && a[i] == abstain_label;
+            if (!abst)
+                ++answering;
+            if (w && !(abst && abstain_policy == 2))
+                st += (double)w[i];
+        }
+        const int32_t k = abstain_policy == 2 ? answering : E;
+        const int by_weight = conf_mode == 2 && st > 0.0;
+        int32_t mode = abstain_label, count = 0;
+        double s_mode = 0.0;
+        int found = 0;
+        for (int32_t i = 0; i < E; ++i) {
+            if (abstain_policy != 0 && a[i] == abstain_label)
+                continue;
+            const int32_t x = a[i];
+            int32_t n = 0;
+            double s = 0.0;
+            for (int32_t j = 0; j < E; ++j) {
+                if (a[j] == x) { /* x is not the sentinel, so expert j answers */
+                    ++n;
+                    if (w)
+                        s += (double)w[j];
+                }
+            }
+            int better;
+            if (!found)
+                better = 1;
+            else if (by_weight)
+                better = s > s_mode || (s == s_mode && x < mode);
+            else
+                better = n > count || (n == count && x < mode);
+            if (better) {
+                found = 1;
+                mode = x;
+                count = n;
+                s_mode = s;
+            }
+        }
+        const float agree = k > 0 ? (float)count / (float)k : 0.0f;
+        float conf = agree;
+        if (conf_mode != 0 && st > 0.0)
+            conf = (float)(s_mode / st);
+        const float t = tau_q ? tau_q[q] : tau;
+        if (mode_out) mode_out[q] = mode;
+        if (count_out) count_out[q] = count;
+        if (agree_out) agree_out[q] = agree;
+        if (conf_out) conf_out[q] = conf;
+        bypass_out[q] = (uint8_t)(conf >= t);
+    }
+}
