@@ -435,6 +435,70 @@ def bench_lse_merge(torch, mosaic, pk, T, Hq, D):
                    static_traffic("lse_merge_dram_bytes_per_launch"))
 
 
+def bench_lse_merge_n(torch, mosaic, pk, T, Hq, D, n=4):
+    """mosaic_lse_merge_n on n = 4 partial results of configs[1]'s shape.
+    Algorithmic bytes: n bf16 reads and one write per element of O, n + 1 fp32 LSE values per row."""
+    dev = "cuda"
+    g = torch.Generator(device=dev).manual_seed(62)
+    op = torch.randn((n, T, Hq, D), device=dev, generator=g).to(torch.bfloat16)
+    lp = torch.randn((n, Hq, T), device=dev, generator=g)
+    o = torch.empty((T, Hq, D), dtype=torch.bfloat16, device=dev)
+    lse = torch.empty((Hq, T), dtype=torch.float32, device=dev)
+    ms = timed(torch, lambda: mosaic.lse_merge_n(op, lp, o=o, lse=lse), 20)   # 5.7 GB: cold
+    return hbm_leg(ms, 2.0 * (n + 1) * T * Hq * D + 4.0 * (n + 1) * T * Hq, pk)
+
+
+def bench_prefix(torch, mosaic, pk):
+    """mosaic_agg_prefill_attn_shared_prefix, 64 contexts of a shared 2048-token block
+    + U{2048..8192} own tokens, Hq/Hkv/D = 28/4/128.  Algorithmic flops: 4 Hq D per visible (row, key)
+    pair = sum_s L_s (L_s + 1) / 2 + T P.  Parity: tests/test_gpu_cascade.py."""
+    n, P_, Hq, Hkv, D = 64, 2048, 28, 4, 128
+    L = np.random.default_rng(91).integers(2048, 8193, size=n).astype(np.int64)
+    cu = np.concatenate([[0], np.cumsum(L)]).astype(np.int64)
+    T = int(cu[-1])
+    dev = "cuda"
+    g = torch.Generator(device=dev).manual_seed(91)
+    q = torch.randn((T, Hq, D), device=dev, generator=g).to(torch.bfloat16)
+    k = torch.randn((T, Hkv, D), device=dev, generator=g).to(torch.bfloat16)
+    v = torch.randn((T, Hkv, D), device=dev, generator=g).to(torch.bfloat16)
+    kp = torch.randn((P_, Hkv, D), device=dev, generator=g).to(torch.bfloat16)
+    vp = torch.randn((P_, Hkv, D), device=dev, generator=g).to(torch.bfloat16)
+    o = torch.empty_like(q)
+    lse = torch.empty((Hq, T), dtype=torch.float32, device=dev)
+    ws = torch.empty(int(mosaic.load().mosaic_agg_prefill_attn_shared_prefix_workspace_bytes(
+        n, T, Hq, Hkv, D)), dtype=torch.uint8, device=dev)
+    cu_d = torch.from_numpy(cu).to(dev)
+    call = lambda: mosaic.agg_prefill_attn_shared_prefix(q, kp, vp, k, v, cu_d, n, int(L.max()),
+                                                         D ** -0.5, o=o, lse=lse, workspace=ws)
+    ms = timed(torch, call, 5)
+    pairs = float(np.sum(L.astype(np.float64) * (L + 1.0) / 2.0) + float(T) * P_)
+    leg = tensor_leg(ms, 4.0 * Hq * D * pairs, pk)
+    leg["tokens"] = T
+    return leg
+
+
+def bench_chunked(torch, mosaic, pk):
+    """mosaic_agg_prefill_attn_chunked, 4 contexts of 45 312 tokens (the longest
+    configs[2] allows) in chunks of 8192 rows, Hq/Hkv/D = 28/4/128, one launch."""
+    n, Lmax, Hq, Hkv, D = 4, 45312, 28, 4, 128
+    cu = np.arange(0, (n + 1) * Lmax, Lmax, dtype=np.int64)
+    T = int(cu[-1])
+    dev = "cuda"
+    g = torch.Generator(device=dev).manual_seed(92)
+    q = torch.randn((T, Hq, D), device=dev, generator=g).to(torch.bfloat16)
+    k = torch.randn((T, Hkv, D), device=dev, generator=g).to(torch.bfloat16)
+    v = torch.randn((T, Hkv, D), device=dev, generator=g).to(torch.bfloat16)
+    o = torch.empty_like(q)
+    lse = torch.empty((Hq, T), dtype=torch.float32, device=dev)
+    ws = torch.empty(int(mosaic.load().mosaic_agg_prefill_attn_chunked_workspace_bytes(
+        n, T, 8192, Hq, Hkv, D)), dtype=torch.uint8, device=dev)
+    cu_d = torch.from_numpy(cu).to(dev)
+    call = lambda: mosaic.agg_prefill_attn_chunked(q, k, v, cu_d, n, Lmax, D ** -0.5, 8192, o=o,
+                                                   lse=lse, workspace=ws)
+    ms = timed(torch, call, 4, 1)
+    return tensor_leg(ms, attn_flops([Lmax] * n, Hq, D), pk)
+
+
 def bench_decode(torch, mosaic, pk):
     """mosaic_agg_decode_attn, one new token for each of 64 sequences of
     U{8192..32768} cached keys, Hq/Hkv/D = 32/8/128.  Algorithmic bytes: K and V read once."""
@@ -664,6 +728,8 @@ def run_product(args):
     nxt = {}
     if "lse_merge" in legs:
         nxt["lse_merge"] = bench_lse_merge(torch, mosaic, pk, C2T, C2.Hq, C2.D)
+    if "lse_merge_n" in legs:
+        nxt["lse_merge_n"] = bench_lse_merge_n(torch, mosaic, pk, C2T, C2.Hq, C2.D)
     if "rope" in legs:
         nxt["rope"] = bench_rope(torch, mosaic, pk, C2T, C2.Hq, C2.Hkv, C2.D)
     if "assemble" in legs:
@@ -672,6 +738,10 @@ def run_product(args):
         nxt["decode"] = bench_decode(torch, mosaic, pk)
     if "attn_kv" in legs:
         nxt["attn_kv"] = bench_attn_kv(torch, mosaic, pk)
+    if "prefix" in legs:
+        nxt["shared_prefix"] = bench_prefix(torch, mosaic, pk)
+    if "chunked" in legs:
+        nxt["chunked"] = bench_chunked(torch, mosaic, pk)
     per_config = bench_per_config(torch, mosaic, wl, pk) if "per_config" in legs else {}
     attn_t = float(np.median(attn_ms)) * 1e-3
     attn_tflops = flops / attn_t / 1e12

@@ -265,6 +265,62 @@ mosaic_status_t mosaic_lse_merge(const void* o_a, const float* lse_a, const void
                                  void* o, float* lse, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * mosaic_lse_merge_n -- mosaic_lse_merge for n partial results over pairwise DISJOINT key sets
+ * (the blocks of a split-KV pass): LSE = ln sum_p e^LSE_p, O = sum_p O_p e^(LSE_p - LSE).
+ *   o_parts [dev] bf16 [n_parts, total_tokens, Hq, D] (16-byte aligned), lse_parts [dev] fp32
+ *   [n_parts, Hq, total_tokens]; o, lse: outputs as mosaic_lse_merge (must not alias the inputs).
+ *   n_parts >= 1.  A row all of whose partials are empty (-inf) gets O = 0, LSE = -inf.
+ * ------------------------------------------------------------------------------------------- */
+mosaic_status_t mosaic_lse_merge_n(const void* o_parts, const float* lse_parts, int32_t n_parts,
+                                   int64_t total_tokens, int32_t Hq, int32_t D, void* o, float* lse,
+                                   void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * mosaic_agg_prefill_attn_chunked -- SURVEY.md section 8(f) N2: mosaic_agg_prefill_attn with every
+ * sequence taken in chunks of q_chunk query rows (chunked prefill of the aggregator's long
+ * contexts: 32 k-token window at P:L194, 45 312 tokens possible in configs[2]).  Chunk c of a
+ * sequence is rows [c q_chunk, min(L, (c+1) q_chunk)) against keys [0, that end): each row sees
+ * exactly the keys the plain prefill shows it, so O and LSE are the plain prefill's (same
+ * tolerances); all chunks of all sequences run in ONE launch of the attention kernel.
+ *   q_chunk >= 1 (a multiple of 256 keeps the tiles of the plain prefill); every other argument as
+ *   mosaic_agg_prefill_attn; workspace >= mosaic_agg_prefill_attn_chunked_workspace_bytes(...).
+ * ------------------------------------------------------------------------------------------- */
+size_t mosaic_agg_prefill_attn_chunked_workspace_bytes(int32_t n_seqs, int64_t total_tokens,
+                                                       int32_t q_chunk, int32_t Hq, int32_t Hkv,
+                                                       int32_t D);
+mosaic_status_t mosaic_agg_prefill_attn_chunked(const void* q, const void* k, const void* v,
+                                                const int64_t* cu_seqlens, int32_t n_seqs,
+                                                int64_t total_tokens, int32_t max_seqlen,
+                                                int32_t Hq, int32_t Hkv, int32_t D,
+                                                float softmax_scale, int32_t q_chunk, void* o,
+                                                float* lse, void* workspace,
+                                                size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * mosaic_agg_prefill_attn_shared_prefix -- SURVEY.md section 8(f) N2, the shared-prefix cascade:
+ * one aggregator serves all survivors with a common prompt template in front of every
+ * context (`Aggregator(q, {a_i})`), so the first prefix_len keys of every sequence are the
+ * SAME block.  Sequence s is  prefix ++ own tokens;  the call computes the rows of the own tokens
+ * (the prefix's rows are the same for every sequence and are the caller's, once): row i of
+ * sequence s sees all prefix_len prefix keys and its own keys j <= i.
+ *   q, o [dev] bf16 [total_tokens, Hq, D], k, v [dev] bf16 [total_tokens, Hkv, D], cu_seqlens,
+ *   lse: the sequences' OWN tokens, as mosaic_agg_prefill_attn;
+ *   k_prefix, v_prefix [dev] bf16 [prefix_len, Hkv, D] (16-byte aligned); prefix_len >= 0.
+ * Two passes over the same kernel -- the own keys (causal), and the packed rows of all sequences
+ * as ONE view against the shared block (non-causal), whose K / V are therefore read from HBM once
+ * for the whole batch -- merged exactly through their logsumexps (mosaic_lse_merge).
+ *   workspace >= mosaic_agg_prefill_attn_shared_prefix_workspace_bytes(...): it holds one
+ *   partial O and LSE.  Errors, alignment and asynchrony as mosaic_agg_prefill_attn.
+ * ------------------------------------------------------------------------------------------- */
+size_t mosaic_agg_prefill_attn_shared_prefix_workspace_bytes(int32_t n_seqs, int64_t total_tokens,
+                                                             int32_t Hq, int32_t Hkv, int32_t D);
+mosaic_status_t mosaic_agg_prefill_attn_shared_prefix(
+    const void* q, const void* k_prefix, const void* v_prefix, int32_t prefix_len, const void* k,
+    const void* v, const int64_t* cu_seqlens, int32_t n_seqs, int64_t total_tokens,
+    int32_t max_seqlen, int32_t Hq, int32_t Hkv, int32_t D, float softmax_scale, void* o, float* lse,
+    void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * mosaic_agg_decode_attn -- SURVEY.md section 8(f) N2: the aggregator's GQA decode attention, one
  * new q token per sequence against all Lk cached keys of that sequence (decode follows prefill in
  * the aggregator): O[s,h,:] = softmax_j(scale q_{s,h} . k_{j,g(h)}) V, LSE as north_star.

@@ -224,6 +224,46 @@ def lse_merge(o_a, lse_a, o_b, lse_b):
     return o, lse
 
 
+def lse_merge_n(o_parts, lse_parts):
+    """the n-way form of lse_merge (reading N2-2): partial results over n
+    pairwise disjoint key sets -> LSE = ln sum_p e^LSE_p, O = sum_p O_p e^(LSE_p - LSE), binary64.
+    o_parts float64 [n,T,Hq,D], lse_parts float64 [n,Hq,T]; -inf marks an empty partial; a row with
+    no non-empty partial gets O = 0, LSE = -inf."""
+    o_parts = np.asarray(o_parts, np.float64)
+    lp = np.asarray(lse_parts, np.float64)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        m = lp.max(axis=0)
+        z = np.where(np.isneginf(lp), 0.0, np.exp(lp - np.where(np.isneginf(m), 0.0, m))).sum(axis=0)
+        lse = np.where(z > 0, m + np.log(np.where(z > 0, z, 1.0)), -np.inf)
+        w = np.where(np.isneginf(lp), 0.0, np.exp(lp - np.where(np.isneginf(lse), 0.0, lse)))  # [n,Hq,T]
+    wt = np.transpose(w, (0, 2, 1))[..., None]                                     # [n,T,Hq,1]
+    o = np.where(wt != 0, o_parts * wt, 0.0).sum(axis=0)
+    return o, lse
+
+
+def attn_shared_prefix(q, k_prefix, v_prefix, k, v, cu_seqlens, softmax_scale):
+    """SURVEY.md 8(f) N2, shared-prefix cascade (reading N2-5): sequence s is the shared
+    block of P keys followed by its own L_s tokens; the rows computed are those of the own tokens,
+    row i seeing all P prefix keys and its own keys j <= i.  Written as the definition: every
+    sequence's keys are concatenated EXPLICITLY (prefix ++ own) and handed to attn_kv_full with
+    Lq = L_s, Lk = P + L_s (bottom-right alignment: key j visible iff j <= i + P).
+    q uint16 [T,Hq,D]; k_prefix, v_prefix uint16 [P,Hkv,D]; k, v uint16 [T,Hkv,D]."""
+    cu = _c(cu_seqlens, np.int64)
+    kp, vp = _c(k_prefix, np.uint16), _c(v_prefix, np.uint16)
+    k, v = _c(k, np.uint16), _c(v, np.uint16)
+    P = kp.shape[0]
+    ks, vs, ck = [], [], [0]
+    for s_ in range(cu.shape[0] - 1):
+        a, b = int(cu[s_]), int(cu[s_ + 1])
+        if b > a:
+            ks += [kp, k[a:b]]
+            vs += [vp, v[a:b]]
+        ck.append(ck[-1] + ((P + b - a) if b > a else 0))
+    kcat = np.concatenate(ks) if ks else np.zeros((0,) + k.shape[1:], np.uint16)
+    vcat = np.concatenate(vs) if vs else np.zeros((0,) + v.shape[1:], np.uint16)
+    return attn_kv_full(q, kcat, vcat, cu, np.asarray(ck, np.int64), softmax_scale, causal=True)
+
+
 def assemble_context(survivor_idx, cu_seqlens, prompt_tokens, prompt_off, trace_tokens, trace_off,
                      E: int):
     """the survivors' aggregator contexts as one packed token batch.  The

@@ -134,15 +134,37 @@ __device__ __forceinline__ int block_suffix_exclusive(int v, int* warp_tot /* [3
     return above + x - v;
 }
 
+// A sequence's q rows and keys come either from the two cu_seqlens arrays (rows / keys of
+// sequence s = [cu[s], cu[s+1])) or, when `desc` is given, from explicit per-sequence views -- q
+// rows and key ranges that need not be adjacent or disjoint (the chunks of a chunked prefill all
+// start at their sequence's first key).
+__device__ __forceinline__ void seq_view(const int64_t* cu_q, const int64_t* cu_k, const SeqDesc* desc,
+                                         int s, int64_t& q0, int64_t& L, int64_t& k0, int64_t& Lk) {
+    if (desc) {
+        const SeqDesc d = desc[s];
+        q0 = d.q_start;
+        L = d.q_len;
+        k0 = d.k_start;
+        Lk = d.k_len;
+    } else {
+        q0 = cu_q[s];
+        L = cu_q[s + 1] - q0;
+        k0 = cu_k[s];
+        Lk = cu_k[s + 1] - k0;
+    }
+}
+
 __global__ void __launch_bounds__(1024) schedule_kernel(const int64_t* __restrict__ cu_seqlens,
                                                         const int64_t* __restrict__ cu_seqlens_k,
+                                                        const SeqDesc* __restrict__ desc,
                                                         int n_seqs, int levels, SchedHeader* header,
                                                         int* cnt, int* start, int* cursor,
                                                         int4* items, int* items_lk) {
     __shared__ int warp_tot[32];
     const int tid = threadIdx.x;
     for (int s = tid; s < n_seqs; s += blockDim.x) {
-        const int64_t L = cu_seqlens[s + 1] - cu_seqlens[s];
+        int64_t q0, L, k0, Lk;
+        seq_view(cu_seqlens, cu_seqlens_k, desc, s, q0, L, k0, Lk);
         const int nb = (int)((L + BQ - 1) / BQ);
         if (nb > 0) atomicAdd(&cnt[min(nb, levels) - 1], 1);
     }
@@ -168,15 +190,13 @@ __global__ void __launch_bounds__(1024) schedule_kernel(const int64_t* __restric
     if (tid == 0) header->n_items = pos;  // thread 0 owns level 0: pos = all entries
     __syncthreads();
     for (int s = tid; s < n_seqs; s += blockDim.x) {
-        const int64_t L = cu_seqlens[s + 1] - cu_seqlens[s];
+        int64_t q0, L, k0, Lk;
+        seq_view(cu_seqlens, cu_seqlens_k, desc, s, q0, L, k0, Lk);
         const int nb = min((int)((L + BQ - 1) / BQ), levels);
-        const int t0 = (int)cu_seqlens[s];  // total_tokens < 2^31
-        const int tk0 = (int)cu_seqlens_k[s];
-        const int Lk = (int)(cu_seqlens_k[s + 1] - cu_seqlens_k[s]);
         for (int c = 0; c < nb; ++c) {
             const int at = start[c] + atomicAdd(&cursor[c], 1);
-            items[at] = make_int4(t0, (int)L, c, tk0);  // everything a CTA needs
-            items_lk[at] = Lk;
+            items[at] = make_int4((int)q0, (int)L, c, (int)k0);  // (token counts are < 2^31)
+            items_lk[at] = (int)Lk;
         }
     }
 }
@@ -916,11 +936,13 @@ extern "C" size_t mosaic_agg_prefill_attn_workspace_bytes(int32_t n_seqs, int64_
     return carve(nullptr, n_seqs, total_tokens).total_bytes;
 }
 
-namespace {
+namespace mosaic {
 // q rows and keys may be packed separately (cu_seqlens / total_tokens for q, O and LSE;
-// cu_seqlens_k / total_k_tokens for K and V); the plain prefill passes the same for both.
+// cu_seqlens_k / total_k_tokens for K and V); the plain prefill passes the same for both.  With
+// `desc` (device array of n_seqs views) the two cu arrays are not read.
 mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int64_t* cu_seqlens,
-                          const int64_t* cu_seqlens_k, int32_t n_seqs, int64_t total_tokens,
+                          const int64_t* cu_seqlens_k, const SeqDesc* desc, int32_t n_seqs,
+                          int64_t total_tokens,
                           int64_t total_k_tokens, int32_t max_seqlen, int32_t Hq, int32_t Hkv,
                           int32_t D, float softmax_scale, int causal, void* o, float* lse,
                           void* workspace, size_t workspace_bytes, void* cuda_stream) {
@@ -930,7 +952,8 @@ mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int
         return MOSAIC_ERR_INVALID_ARG;
     if (D != 64 && D != 128) return MOSAIC_ERR_UNSUPPORTED;
     if (n_seqs == 0 || total_tokens == 0) return MOSAIC_OK;
-    if (!q || !k || !v || !o || !lse || !cu_seqlens || !cu_seqlens_k || !workspace || !aligned16(q) ||
+    if (!q || !k || !v || !o || !lse || (!desc && (!cu_seqlens || !cu_seqlens_k)) || !workspace ||
+        !aligned16(q) ||
         !aligned16(k) || !aligned16(v) || !aligned16(o) || !aligned16(workspace))
         return MOSAIC_ERR_INVALID_ARG;
     Workspace w = carve(workspace, n_seqs, total_tokens);
@@ -945,8 +968,8 @@ mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int
 
     const int levels = (int)(total_tokens / BQ) + 2;
     MOSAIC_CUDA_TRY(cudaMemsetAsync(workspace, 0, w.zero_bytes, s));
-    schedule_kernel<<<1, 1024, 0, s>>>(cu_seqlens, cu_seqlens_k, n_seqs, levels, w.header, w.cnt,
-                                       w.start, w.cursor, w.items, w.items_lk);
+    schedule_kernel<<<1, 1024, 0, s>>>(cu_seqlens, cu_seqlens_k, desc, n_seqs, levels, w.header,
+                                       w.cnt, w.start, w.cursor, w.items, w.items_lk);
     count_launch();
     MOSAIC_CUDA_TRY(cudaGetLastError());
 
@@ -971,7 +994,7 @@ mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int
     return D == 64 ? launch_attn<64>(tq, tk, tv, p, negate_q, grid, s)
                    : launch_attn<128>(tq, tk, tv, p, negate_q, grid, s);
 }
-}  // namespace
+}  // namespace mosaic
 
 extern "C" mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k, const void* v,
                                                    const int64_t* cu_seqlens, int32_t n_seqs,
@@ -980,7 +1003,7 @@ extern "C" mosaic_status_t mosaic_agg_prefill_attn(const void* q, const void* k,
                                                    float softmax_scale, void* o, float* lse,
                                                    void* workspace, size_t workspace_bytes,
                                                    void* cuda_stream) {
-    return attn_impl(q, k, v, cu_seqlens, cu_seqlens, n_seqs, total_tokens, total_tokens, max_seqlen,
+    return attn_impl(q, k, v, cu_seqlens, cu_seqlens, nullptr, n_seqs, total_tokens, total_tokens, max_seqlen,
                      Hq, Hkv, D, softmax_scale, 1, o, lse, workspace, workspace_bytes, cuda_stream);
 }
 
@@ -989,7 +1012,7 @@ extern "C" mosaic_status_t mosaic_agg_prefill_attn_kv(
     const int64_t* cu_seqlens_k, int32_t n_seqs, int64_t total_q_tokens, int64_t total_k_tokens,
     int32_t max_seqlen_q, int32_t Hq, int32_t Hkv, int32_t D, float softmax_scale, int32_t causal,
     void* o, float* lse, void* workspace, size_t workspace_bytes, void* cuda_stream) {
-    return attn_impl(q, k, v, cu_seqlens_q, cu_seqlens_k, n_seqs, total_q_tokens, total_k_tokens,
+    return attn_impl(q, k, v, cu_seqlens_q, cu_seqlens_k, nullptr, n_seqs, total_q_tokens, total_k_tokens,
                      max_seqlen_q, Hq, Hkv, D, softmax_scale, causal, o, lse, workspace,
                      workspace_bytes, cuda_stream);
 }

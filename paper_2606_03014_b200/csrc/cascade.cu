@@ -1,0 +1,198 @@
+// cascade.cu -- SURVEY.md section 8(f) N2, the LSE-merge variants built on the prefill kernel:
+//   mosaic_agg_prefill_attn_chunked        chunked prefill of long contexts (32 k-class
+//                                          windows; configs[2] allows 45 312 tokens) in ONE launch
+//   mosaic_agg_prefill_attn_shared_prefix  shared-prefix cascade: every survivor's context starts
+//                                          with the same block of keys (the aggregator's prompt
+//                                          template, P:L225 / P:L377 `Aggregator(q, {a_i})`)
+// Only plans, descriptors and the order of calls live here; the attention is attn.cu's kernel and
+// the merge is merge.cu's.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include "common.cuh"
+
+namespace mosaic {
+namespace {
+
+inline size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
+
+// ---- chunked prefill: chunk c of sequence s is a view of its own -- q rows [c C, min(L, (c+1) C))
+// of the sequence against keys [0, that end): the bottom-right alignment of reading N2-1, so the
+// rows see exactly the keys the plain prefill shows them.  One block: chunks per sequence, their
+// exclusive scan, one descriptor per chunk, empty descriptors in the unused tail.
+__global__ void __launch_bounds__(1024) chunk_plan_kernel(const int64_t* __restrict__ cu_seqlens,
+                                                          int n_seqs, int q_chunk, int64_t v_max,
+                                                          SeqDesc* __restrict__ desc) {
+    __shared__ int warp_tot[32];
+    __shared__ int carry;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) carry = 0;
+    __syncthreads();
+    for (int s0 = 0; s0 < n_seqs; s0 += 1024) {
+        const int s = s0 + tid;
+        int64_t t0 = 0, L = 0;
+        if (s < n_seqs) {
+            t0 = cu_seqlens[s];
+            L = cu_seqlens[s + 1] - t0;
+        }
+        const int nc = (int)((L + q_chunk - 1) / q_chunk);
+        int x = nc;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_tot[warp] = x;
+        __syncthreads();
+        int before = carry;
+        for (int w = 0; w < warp; ++w) before += warp_tot[w];
+        const int first = before + x - nc;
+        for (int c = 0; c < nc; ++c) {
+            const int64_t r0 = (int64_t)c * q_chunk;
+            const int64_t r1 = min(L, r0 + q_chunk);
+            desc[first + c] = SeqDesc{t0 + r0, t0, (int32_t)(r1 - r0), (int32_t)r1};
+        }
+        __syncthreads();
+        if (tid == 1023) carry = before + x;
+        __syncthreads();
+    }
+    for (int64_t v = carry + tid; v < v_max; v += 1024) desc[v] = SeqDesc{0, 0, 0, 0};
+}
+
+// ---- shared prefix: the packed q rows of ALL sequences as one view against the prefix block
+__global__ void prefix_view_kernel(SeqDesc* desc, int64_t T, int32_t P) {
+    desc[0] = SeqDesc{0, 0, (int32_t)T, P};
+}
+
+struct ChunkWs {
+    SeqDesc* desc;
+    void* attn_ws;
+    size_t attn_ws_bytes, total;
+    int64_t v_max;
+};
+ChunkWs carve_chunked(void* base, int32_t n_seqs, int64_t total_tokens, int32_t q_chunk, int32_t Hq,
+                      int32_t Hkv, int32_t D) {
+    ChunkWs w{};
+    w.v_max = total_tokens / q_chunk + n_seqs;
+    char* p = static_cast<char*>(base);
+    size_t off = 0;
+    w.desc = reinterpret_cast<SeqDesc*>(p + off);
+    off += align256((size_t)w.v_max * sizeof(SeqDesc));
+    w.attn_ws_bytes = mosaic_agg_prefill_attn_workspace_bytes(
+        (int32_t)(w.v_max < (1ll << 31) - 1 ? w.v_max : (1ll << 31) - 1), total_tokens, Hq, Hkv, D);
+    w.attn_ws = p + off;
+    off += align256(w.attn_ws_bytes);
+    w.total = off;
+    return w;
+}
+
+struct PrefixWs {
+    SeqDesc* desc;
+    void* o_tmp;
+    float* lse_tmp;
+    void* attn_ws;
+    size_t attn_ws_bytes, total;
+};
+PrefixWs carve_prefix(void* base, int32_t n_seqs, int64_t total_tokens, int32_t Hq, int32_t Hkv,
+                      int32_t D) {
+    PrefixWs w{};
+    char* p = static_cast<char*>(base);
+    size_t off = 0;
+    w.desc = reinterpret_cast<SeqDesc*>(p + off);
+    off += 256;
+    w.o_tmp = p + off;
+    off += align256((size_t)total_tokens * Hq * D * 2);
+    w.lse_tmp = reinterpret_cast<float*>(p + off);
+    off += align256((size_t)total_tokens * Hq * 4);
+    // the larger of the two passes' work lists: one view of T rows, n_seqs views of T rows together
+    w.attn_ws_bytes = mosaic_agg_prefill_attn_workspace_bytes(n_seqs > 1 ? n_seqs : 1, total_tokens,
+                                                              Hq, Hkv, D);
+    w.attn_ws = p + off;
+    off += align256(w.attn_ws_bytes);
+    w.total = off;
+    return w;
+}
+
+}  // namespace
+}  // namespace mosaic
+
+using namespace mosaic;
+
+extern "C" size_t mosaic_agg_prefill_attn_chunked_workspace_bytes(int32_t n_seqs,
+                                                                  int64_t total_tokens,
+                                                                  int32_t q_chunk, int32_t Hq,
+                                                                  int32_t Hkv, int32_t D) {
+    if (n_seqs < 0 || total_tokens < 0 || q_chunk < 1) return 0;
+    return carve_chunked(nullptr, n_seqs, total_tokens, q_chunk, Hq, Hkv, D).total;
+}
+
+extern "C" mosaic_status_t mosaic_agg_prefill_attn_chunked(
+    const void* q, const void* k, const void* v, const int64_t* cu_seqlens, int32_t n_seqs,
+    int64_t total_tokens, int32_t max_seqlen, int32_t Hq, int32_t Hkv, int32_t D,
+    float softmax_scale, int32_t q_chunk, void* o, float* lse, void* workspace,
+    size_t workspace_bytes, void* cuda_stream) {
+    if (n_seqs < 0 || total_tokens < 0 || total_tokens >= (1ll << 31) || max_seqlen < 0 ||
+        q_chunk < 1 || Hq < 1 || Hkv < 1 || Hq % Hkv != 0 || !isfinite(softmax_scale))
+        return MOSAIC_ERR_INVALID_ARG;
+    if (D != 64 && D != 128) return MOSAIC_ERR_UNSUPPORTED;
+    if (n_seqs == 0 || total_tokens == 0) return MOSAIC_OK;
+    if (!cu_seqlens || !workspace || !aligned16(workspace)) return MOSAIC_ERR_INVALID_ARG;
+    ChunkWs w = carve_chunked(workspace, n_seqs, total_tokens, q_chunk, Hq, Hkv, D);
+    if (workspace_bytes < w.total) return MOSAIC_ERR_WORKSPACE_TOO_SMALL;
+    if (w.v_max >= (1ll << 31) - 1) return MOSAIC_ERR_UNSUPPORTED;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    chunk_plan_kernel<<<1, 1024, 0, s>>>(cu_seqlens, n_seqs, q_chunk, w.v_max, w.desc);
+    count_launch();
+    MOSAIC_CUDA_TRY(cudaGetLastError());
+    return attn_impl(q, k, v, nullptr, nullptr, w.desc, (int32_t)w.v_max, total_tokens, total_tokens,
+                     q_chunk < max_seqlen ? q_chunk : max_seqlen, Hq, Hkv, D, softmax_scale,
+                     /*causal=*/1, o, lse, w.attn_ws, w.attn_ws_bytes, cuda_stream);
+}
+
+extern "C" size_t mosaic_agg_prefill_attn_shared_prefix_workspace_bytes(int32_t n_seqs,
+                                                                        int64_t total_tokens,
+                                                                        int32_t Hq, int32_t Hkv,
+                                                                        int32_t D) {
+    if (n_seqs < 0 || total_tokens < 0 || Hq < 1 || Hkv < 1 || D < 1) return 0;
+    return carve_prefix(nullptr, n_seqs, total_tokens, Hq, Hkv, D).total;
+}
+
+extern "C" mosaic_status_t mosaic_agg_prefill_attn_shared_prefix(
+    const void* q, const void* k_prefix, const void* v_prefix, int32_t prefix_len, const void* k,
+    const void* v, const int64_t* cu_seqlens, int32_t n_seqs, int64_t total_tokens,
+    int32_t max_seqlen, int32_t Hq, int32_t Hkv, int32_t D, float softmax_scale, void* o,
+    float* lse, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (n_seqs < 0 || total_tokens < 0 || total_tokens >= (1ll << 31) || max_seqlen < 0 ||
+        prefix_len < 0 || Hq < 1 || Hkv < 1 || Hq % Hkv != 0 || !isfinite(softmax_scale))
+        return MOSAIC_ERR_INVALID_ARG;
+    if (D != 64 && D != 128) return MOSAIC_ERR_UNSUPPORTED;
+    if (n_seqs == 0 || total_tokens == 0) return MOSAIC_OK;
+    if (!workspace || !aligned16(workspace)) return MOSAIC_ERR_INVALID_ARG;
+    PrefixWs w = carve_prefix(workspace, n_seqs, total_tokens, Hq, Hkv, D);
+    if (workspace_bytes < w.total) return MOSAIC_ERR_WORKSPACE_TOO_SMALL;
+    // the sequences' own keys: the plain causal prefill over the suffixes
+    if (prefix_len == 0)
+        return mosaic_agg_prefill_attn(q, k, v, cu_seqlens, n_seqs, total_tokens, max_seqlen, Hq, Hkv,
+                                       D, softmax_scale, o, lse, w.attn_ws, w.attn_ws_bytes,
+                                       cuda_stream);
+    if (!k_prefix || !v_prefix || !aligned16(k_prefix) || !aligned16(v_prefix))
+        return MOSAIC_ERR_INVALID_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    mosaic_status_t st = mosaic_agg_prefill_attn(q, k, v, cu_seqlens, n_seqs, total_tokens, max_seqlen,
+                                                 Hq, Hkv, D, softmax_scale, w.o_tmp, w.lse_tmp,
+                                                 w.attn_ws, w.attn_ws_bytes, cuda_stream);
+    if (st != MOSAIC_OK) return st;
+    // the shared block: every q row of every sequence sees all of it, so the packed rows are ONE
+    // view of total_tokens rows against prefix_len keys -- 128-row tiles run across the sequence
+    // boundaries and the block's K / V tiles (a few MB: L2-resident) are read from HBM once
+    prefix_view_kernel<<<1, 1, 0, s>>>(w.desc, total_tokens, prefix_len);
+    count_launch();
+    MOSAIC_CUDA_TRY(cudaGetLastError());
+    st = attn_impl(q, k_prefix, v_prefix, nullptr, nullptr, w.desc, 1, total_tokens, prefix_len,
+                   max_seqlen, Hq, Hkv, D, softmax_scale, /*causal=*/0, o, lse, w.attn_ws,
+                   w.attn_ws_bytes, cuda_stream);
+    if (st != MOSAIC_OK) return st;
+    // disjoint key sets: merged exactly through the logsumexps (reading N2-2), in place
+    return mosaic_lse_merge(o, lse, w.o_tmp, w.lse_tmp, total_tokens, Hq, D, o, lse, cuda_stream);
+}

@@ -29,6 +29,20 @@ inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 
 constexpr int kNumSMsB200 = 148;
 
+// One sequence of an attention call as explicit views (attn.cu: attn_impl with `desc`): q rows
+// [q_start, q_start + q_len) of the packed q / o / lse, keys [k_start, k_start + k_len) of k / v.
+struct SeqDesc {
+    int64_t q_start, k_start;
+    int32_t q_len, k_len;
+};
+// The attention behind mosaic_agg_prefill_attn[_kv] (attn.cu), for the entry points built on it.
+mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int64_t* cu_seqlens,
+                          const int64_t* cu_seqlens_k, const SeqDesc* desc, int32_t n_seqs,
+                          int64_t total_tokens, int64_t total_k_tokens, int32_t max_seqlen,
+                          int32_t Hq, int32_t Hkv, int32_t D, float softmax_scale, int causal,
+                          void* o, float* lse, void* workspace, size_t workspace_bytes,
+                          void* cuda_stream);
+
 // Number of SMs of the current device (cached per thread; 148 on B200).
 int num_sms();
 

@@ -95,3 +95,74 @@ extern "C" mosaic_status_t mosaic_lse_merge(const void* o_a, const float* lse_a,
     MOSAIC_CUDA_TRY(cudaGetLastError());
     return MOSAIC_OK;
 }
+
+// ------------------------------------------------------------------------------------------
+// mosaic_lse_merge_n: the same merge for n partial results at once (the chunks of a split-KV
+// pass): LSE = ln sum_p e^LSE_p, O = sum_p O_p e^(LSE_p - LSE).  A thread takes 8 consecutive
+// elements of one (token, head) row and walks the n parts twice (the row's n logsumexps for the
+// maximum, then the weighted sum in fp32): every O_p element is read once.
+namespace mosaic {
+namespace {
+__global__ void __launch_bounds__(kMergeThreads) lse_merge_n_kernel(
+    const __nv_bfloat16* __restrict__ o_parts, const float* __restrict__ lse_parts, int n_parts,
+    int64_t T, int Hq, int D, __nv_bfloat16* __restrict__ o, float* __restrict__ lse) {
+    const int per_row = D / 8;
+    const int64_t gid = (int64_t)blockIdx.x * kMergeThreads + threadIdx.x;
+    const int64_t rowi = gid / per_row;  // (token, head) row
+    if (rowi >= T * Hq) return;
+    const int c = (int)(gid - rowi * per_row);
+    const int64_t t = rowi / Hq;
+    const int h = (int)(rowi - t * Hq);
+    const int64_t o_stride = T * (int64_t)Hq * D, l_stride = (int64_t)Hq * T;
+    const float* lrow = lse_parts + (int64_t)h * T + t;
+    float m = -INFINITY;
+    for (int p = 0; p < n_parts; ++p) m = fmaxf(m, lrow[p * l_stride]);
+    float acc[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) acc[u] = 0.f;
+    float z = 0.f;
+    if (m > -INFINITY) {
+        for (int p = 0; p < n_parts; ++p) {
+            const float l = lrow[p * l_stride];
+            if (l == -INFINITY) continue;  // an empty partial: weight 0, its O is not read
+            const float w = expf(l - m);
+            z += w;
+            const uint4 v = *reinterpret_cast<const uint4*>(o_parts + p * o_stride + rowi * D + c * 8);
+            const __nv_bfloat162* pv = reinterpret_cast<const __nv_bfloat162*>(&v);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const float2 f = __bfloat1622float2(pv[u]);
+                acc[2 * u] = fmaf(f.x, w, acc[2 * u]);
+                acc[2 * u + 1] = fmaf(f.y, w, acc[2 * u + 1]);
+            }
+        }
+    }
+    const float inv = z > 0.f ? 1.f / z : 0.f;
+    uint4 out;
+    __nv_bfloat162* po = reinterpret_cast<__nv_bfloat162*>(&out);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) po[u] = __floats2bfloat162_rn(acc[2 * u] * inv, acc[2 * u + 1] * inv);
+    *reinterpret_cast<uint4*>(o + rowi * D + c * 8) = out;
+    if (c == 0) lse[(int64_t)h * T + t] = z > 0.f ? m + logf(z) : -INFINITY;
+}
+}  // namespace
+}  // namespace mosaic
+
+extern "C" mosaic_status_t mosaic_lse_merge_n(const void* o_parts, const float* lse_parts,
+                                              int32_t n_parts, int64_t total_tokens, int32_t Hq,
+                                              int32_t D, void* o, float* lse, void* cuda_stream) {
+    if (n_parts < 1 || total_tokens < 0 || Hq < 1 || D < 8 || D % 8 != 0)
+        return MOSAIC_ERR_INVALID_ARG;
+    if (total_tokens == 0) return MOSAIC_OK;
+    if (!o_parts || !lse_parts || !o || !lse || !aligned16(o_parts) || !aligned16(o))
+        return MOSAIC_ERR_INVALID_ARG;
+    const int64_t threads = total_tokens * Hq * (D / 8);
+    const int64_t blocks = (threads + kMergeThreads - 1) / kMergeThreads;
+    if (blocks >= (1ll << 31)) return MOSAIC_ERR_UNSUPPORTED;
+    lse_merge_n_kernel<<<(unsigned)blocks, kMergeThreads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        static_cast<const __nv_bfloat16*>(o_parts), lse_parts, n_parts, total_tokens, Hq, D,
+        static_cast<__nv_bfloat16*>(o), lse);
+    count_launch();
+    MOSAIC_CUDA_TRY(cudaGetLastError());
+    return MOSAIC_OK;
+}

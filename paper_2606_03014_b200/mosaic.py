@@ -45,6 +45,15 @@ SIGNATURES = {
     "mosaic_agg_decode_attn": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i64, _i32, _i32, _i32, _f32,
                                               _vp, _vp, _vp, _sz, _vp]),
     "mosaic_lse_merge": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i64, _i32, _i32, _vp, _vp, _vp]),
+    "mosaic_lse_merge_n": (ctypes.c_int, [_vp, _vp, _i32, _i64, _i32, _i32, _vp, _vp, _vp]),
+    "mosaic_agg_prefill_attn_chunked_workspace_bytes": (_sz, [_i32, _i64, _i32, _i32, _i32, _i32]),
+    "mosaic_agg_prefill_attn_chunked": (ctypes.c_int, [_vp, _vp, _vp, _vp, _i32, _i64, _i32, _i32,
+                                                       _i32, _i32, _f32, _i32, _vp, _vp, _vp, _sz,
+                                                       _vp]),
+    "mosaic_agg_prefill_attn_shared_prefix_workspace_bytes": (_sz, [_i32, _i64, _i32, _i32, _i32]),
+    "mosaic_agg_prefill_attn_shared_prefix": (ctypes.c_int, [_vp, _vp, _vp, _i32, _vp, _vp, _vp, _i32,
+                                                             _i64, _i32, _i32, _i32, _i32, _f32, _vp,
+                                                             _vp, _vp, _sz, _vp]),
     "mosaic_assemble_context": (ctypes.c_int, [_vp, _vp, _i32, _i32, _vp, _vp, _vp, _vp, _i32, _vp,
                                                _vp, _vp, _vp]),
     "mosaic_rope_packed": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _i32, _i32, _f32, _vp]),
@@ -340,6 +349,70 @@ def lse_merge(o_a, lse_a, o_b, lse_b, *, o=None, lse=None, stream=None):
                                  int(T), Hq, D, _dptr(o, torch.bfloat16, "o"),
                                  _dptr(lse, torch.float32, "lse"), _stream(stream))
     _check("mosaic_lse_merge", st)
+    return o, lse
+
+
+def lse_merge_n(o_parts, lse_parts, *, o=None, lse=None, stream=None):
+    """mosaic_lse_merge_n: o_parts bf16 [n, T, Hq, D], lse_parts fp32 [n, Hq, T] -> (o, lse)."""
+    n, T, Hq, D = o_parts.shape
+    if o is None:
+        o = torch.empty((T, Hq, D), dtype=torch.bfloat16, device=o_parts.device)
+    if lse is None:
+        lse = torch.empty((Hq, T), dtype=torch.float32, device=o_parts.device)
+    st = load().mosaic_lse_merge_n(_dptr(o_parts, torch.bfloat16, "o_parts"),
+                                   _dptr(lse_parts, torch.float32, "lse_parts"), int(n), int(T), Hq, D,
+                                   _dptr(o, torch.bfloat16, "o"), _dptr(lse, torch.float32, "lse"),
+                                   _stream(stream))
+    _check("mosaic_lse_merge_n", st)
+    return o, lse
+
+
+def agg_prefill_attn_chunked(q, k, v, cu_seqlens, n_seqs, max_seqlen, softmax_scale, q_chunk, *,
+                             o=None, lse=None, workspace=None, stream=None):
+    """mosaic_agg_prefill_attn_chunked: the plain prefill with every sequence taken in chunks of
+    q_chunk query rows, all chunks in one launch."""
+    T, Hq, D = q.shape
+    Hkv = k.shape[1]
+    dev = q.device
+    if o is None:
+        o = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty((Hq, T), dtype=torch.float32, device=dev)
+    if workspace is None:
+        nb = int(load().mosaic_agg_prefill_attn_chunked_workspace_bytes(int(n_seqs), T, int(q_chunk),
+                                                                        Hq, Hkv, D))
+        workspace = torch.empty(max(nb, 16), dtype=torch.uint8, device=dev)
+    st = load().mosaic_agg_prefill_attn_chunked(
+        _dptr(q, torch.bfloat16, "q"), _dptr(k, torch.bfloat16, "k"), _dptr(v, torch.bfloat16, "v"),
+        _dptr(cu_seqlens, torch.int64, "cu_seqlens"), int(n_seqs), int(T), int(max_seqlen), Hq, Hkv, D,
+        float(softmax_scale), int(q_chunk), _dptr(o, torch.bfloat16, "o"),
+        _dptr(lse, torch.float32, "lse"), _dptr(workspace), workspace.numel(), _stream(stream))
+    _check("mosaic_agg_prefill_attn_chunked", st)
+    return o, lse
+
+
+def agg_prefill_attn_shared_prefix(q, k_prefix, v_prefix, k, v, cu_seqlens, n_seqs, max_seqlen,
+                                   softmax_scale, *, o=None, lse=None, workspace=None, stream=None):
+    """mosaic_agg_prefill_attn_shared_prefix: every sequence = the shared block k_prefix / v_prefix
+    bf16 [P, Hkv, D] followed by its own tokens (q, k, v packed by cu_seqlens)."""
+    T, Hq, D = q.shape
+    Hkv = k.shape[1]
+    P = 0 if k_prefix is None else k_prefix.shape[0]
+    dev = q.device
+    if o is None:
+        o = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty((Hq, T), dtype=torch.float32, device=dev)
+    if workspace is None:
+        nb = int(load().mosaic_agg_prefill_attn_shared_prefix_workspace_bytes(int(n_seqs), T, Hq, Hkv, D))
+        workspace = torch.empty(max(nb, 16), dtype=torch.uint8, device=dev)
+    st = load().mosaic_agg_prefill_attn_shared_prefix(
+        _dptr(q, torch.bfloat16, "q"), _dptr(k_prefix, torch.bfloat16, "k_prefix"),
+        _dptr(v_prefix, torch.bfloat16, "v_prefix"), int(P), _dptr(k, torch.bfloat16, "k"),
+        _dptr(v, torch.bfloat16, "v"), _dptr(cu_seqlens, torch.int64, "cu_seqlens"), int(n_seqs),
+        int(T), int(max_seqlen), Hq, Hkv, D, float(softmax_scale), _dptr(o, torch.bfloat16, "o"),
+        _dptr(lse, torch.float32, "lse"), _dptr(workspace), workspace.numel(), _stream(stream))
+    _check("mosaic_agg_prefill_attn_shared_prefix", st)
     return o, lse
 
 
