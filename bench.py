@@ -12,7 +12,8 @@ events around its launches) against the measured dense-bf16 peak (the sustained 
 region is seconds long; `frac_burst` is the same against the burst figure).  `gate` is the
 gate+compaction call on the same 2^20 questions against the measured HBM copy bandwidth, L2-cold
 by rotating buffer sets.  `per_config` times the attention of configs[1..4] (C2..C5) alone.
-`next` holds the SURVEY 8(f) legs (shapes in DESIGN.md section 7).  `cpu_baseline` times the fp64
+`next` holds the SURVEY 8(f) legs (shapes in DESIGN.md section 7; `gbs` legs are HBM-bound, against
+the measured copy bandwidth, `tflops` legs tensor-bound).  `cpu_baseline` times the fp64
 oracle on a bounded row sample of the same workload.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--legs a,b,...]
@@ -214,7 +215,7 @@ def oracle_sample(cfg, seed, budget_rows):
 def workload_name(cfg):
     return (f"{cfg.name} (BASELINE.json configs[{cfg.config_id - 1}]): gate+compaction over "
             f"2^20 questions (E=8, weighted conf), attention over the first {cfg.max_attn_seqs} "
-            f"survivors (Hq/Hkv/D={cfg.Hq}/{cfg.Hkv}/{cfg.D}, 8-32 k tokens each)")
+            f"survivors (Hq/Hkv/D={cfg.Hq}/{cfg.Hkv}/{cfg.D}, 8-32 k tokens)")
 
 
 def run_reference(args):
@@ -266,8 +267,7 @@ def timed(torch, fn, n, warm=2):
 def hbm_leg(ms, byts, pk, traffic=None):
     t = float(np.median(ms)) * 1e-3
     return {"us": r3(t * 1e6), "us_best": r3(float(ms.min()) * 1e3), "gbs": r3(byts / t / 1e9),
-            "frac": r3(byts / t / 1e9 / pk["hbm_gbs"]), "bound": "hbm", "bytes": int(byts),
-            "traffic": traffic}
+            "frac": r3(byts / t / 1e9 / pk["hbm_gbs"]), "bytes": int(byts), "traffic": traffic}
 
 
 def tensor_leg(ms, fl, pk):
@@ -278,8 +278,7 @@ def tensor_leg(ms, fl, pk):
     kind = "sustained" if float(ms.sum()) > 300.0 else "burst"
     peak = pk["bf16_tflops_sustained"] if kind == "sustained" else pk["bf16_tflops"]
     return {"ms": r3(t * 1e3), "ms_best": r3(float(ms.min())), "tflop": r3(fl / 1e12),
-            "tflops": r3(fl / t / 1e12), "frac": r3(fl / t / 1e12 / peak), "peak_kind": kind,
-            "bound": "tensor"}
+            "tflops": r3(fl / t / 1e12), "frac": r3(fl / t / 1e12 / peak), "peak_kind": kind}
 
 
 def bench_gate_c5(torch, mosaic, wl, pk, gi, steps=80, warmup=8):
@@ -319,11 +318,11 @@ def bench_gate_c5(torch, mosaic, wl, pk, gi, steps=80, warmup=8):
     ms = timed(torch, graph.replay, max(3, steps // nsets), max(1, warmup // nsets)) / nsets
     t = float(np.median(ms)) * 1e-3
     gbs = byts / t / 1e9
-    return {"workload": "configs[4] gate+compaction: Q=2^20, E=8, weighted conf, p=0.6, tau=0.75",
+    return {"workload": "configs[4]: Q=2^20, E=8, weighted conf, p=0.6, tau=0.75",
             "mqueries_per_s": r3(cfg.Q / t / 1e6), "us_per_call": r3(t * 1e6),
             "us_best": r3(float(ms.min()) * 1e3), "survivors": S,
             "kernels_per_call": int(launches_per_call),
-            "l2": "cold: 4 buffer sets (~93 MB each) round-robin, CUDA-graph replay",
+            "l2": "cold: 4 buffer sets round-robin, CUDA-graph replay",
             "roofline": {"bound": "hbm", "achieved": r3(gbs), "peak": pk["hbm_gbs"], "unit": "GB/s",
                          "frac": r3(gbs / pk["hbm_gbs"]), "frac_of_8tbs": r3(gbs / 8000.0),
                          "traffic": static_traffic("gate_compact_dram_bytes_per_launch"),

@@ -111,11 +111,12 @@ inline Workspace carve(void* base, int32_t n_seqs, int64_t total_tokens) {
     return w;
 }
 
-// Work items in descending cost order.  The cost of (sequence s, q block c) is its number of KV
-// tiles, ~2c + 2, so "longest first" is "descending c": level c holds one entry for every
-// sequence with more than c blocks.  Counting sort over levels; order inside a level is arbitrary
-// (the results do not depend on the schedule).  One block; the two scans over the levels are
-// chunked over its threads.
+// Work items in descending cost order.  The cost of (sequence s, q block c) is the number of KV
+// tiles its rows visit: in 256-key units, level(s, c) = ceil(min(off_s + 256 (c + 1), Lk_s) / 256) - 1
+// with off_s = Lk_s - Lq_s when causal (the plain prefill: level = c), and ceil(Lk_s / 256) - 1 for
+// every block when not.  Counting sort over the levels, highest first; order inside a level is
+// arbitrary (the results do not depend on the schedule).  One block; the scans over the levels
+// are chunked over its threads.
 
 // Sum of v over the threads with a larger thread index (whole block calls).
 __device__ __forceinline__ int block_suffix_exclusive(int v, int* warp_tot /* [32] shared */) {
@@ -132,6 +133,22 @@ __device__ __forceinline__ int block_suffix_exclusive(int v, int* warp_tot /* [3
     int above = 0;
     for (int w = warp + 1; w < nwarp; ++w) above += warp_tot[w];
     return above + x - v;
+}
+// Sum of v over the threads with a smaller thread index (whole block calls).
+__device__ __forceinline__ int block_prefix_exclusive(int v, int* warp_tot /* [32] shared */) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int x = v;  // inclusive prefix inside the warp
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    __syncthreads();
+    if (lane == 31) warp_tot[warp] = x;
+    __syncthreads();
+    int below = 0;
+    for (int w = 0; w < warp; ++w) below += warp_tot[w];
+    return below + x - v;
 }
 
 // A sequence's q rows and keys come either from the two cu_seqlens arrays (rows / keys of
@@ -154,32 +171,68 @@ __device__ __forceinline__ void seq_view(const int64_t* cu_q, const int64_t* cu_
     }
 }
 
+// The levels of a sequence's blocks: block c sits at level lv0 + (causal ? c : 0), clipped.
+__device__ __forceinline__ void seq_levels(int64_t L, int64_t Lk, int causal, int levels, int& nb,
+                                           int& lv0) {
+    nb = (int)((L + BQ - 1) / BQ);
+    if (causal) {
+        const int64_t off = Lk > L ? Lk - L : 0;
+        lv0 = (int)min((int64_t)levels - 1, off / BQ);  // level(c) = floor(off / 256) + c (+ a partial unit)
+    } else {
+        lv0 = (int)min((int64_t)levels - 1, Lk > 0 ? (Lk - 1) / BQ : 0);
+    }
+}
+
 __global__ void __launch_bounds__(1024) schedule_kernel(const int64_t* __restrict__ cu_seqlens,
                                                         const int64_t* __restrict__ cu_seqlens_k,
                                                         const SeqDesc* __restrict__ desc,
-                                                        int n_seqs, int levels, SchedHeader* header,
-                                                        int* cnt, int* start, int* cursor,
-                                                        int4* items, int* items_lk) {
+                                                        int n_seqs, int levels, int causal,
+                                                        SchedHeader* header, int* cnt, int* start,
+                                                        int* cursor, int4* items, int* items_lk) {
     __shared__ int warp_tot[32];
+    __shared__ int lv_min;  // levels are counted from the cheapest block of the batch: the arrays
+                            // hold total_q_tokens / 256 + 2 levels however long the keys are
     const int tid = threadIdx.x;
+    if (tid == 0) lv_min = 0x7fffffff;
+    __syncthreads();
     for (int s = tid; s < n_seqs; s += blockDim.x) {
         int64_t q0, L, k0, Lk;
         seq_view(cu_seqlens, cu_seqlens_k, desc, s, q0, L, k0, Lk);
-        const int nb = (int)((L + BQ - 1) / BQ);
-        if (nb > 0) atomicAdd(&cnt[min(nb, levels) - 1], 1);
+        int nb, lv0;
+        seq_levels(L, Lk, causal, 0x7fffffff, nb, lv0);
+        if (nb > 0) atomicMin(&lv_min, lv0);
+    }
+    __syncthreads();
+    const int base = lv_min == 0x7fffffff ? 0 : lv_min;
+    // cnt[] starts as a difference array: +w at the first level of a sequence's blocks, -w behind
+    // the last (causal: one block per level over nb levels; not causal: nb blocks at one level)
+    for (int s = tid; s < n_seqs; s += blockDim.x) {
+        int64_t q0, L, k0, Lk;
+        seq_view(cu_seqlens, cu_seqlens_k, desc, s, q0, L, k0, Lk);
+        int nb, lv0;
+        seq_levels(L, Lk, causal, 0x7fffffff, nb, lv0);
+        lv0 = min(levels - 1, lv0 - base);
+        if (nb > 0) {
+            const int hi = causal ? min(levels, lv0 + nb) : lv0 + 1;  // (levels past the clip share the top one)
+            const int w = causal ? 1 : nb;
+            atomicAdd(&cnt[lv0], w);
+            if (hi < levels) atomicAdd(&cnt[hi], -w);
+            if (causal && lv0 + nb > levels) atomicAdd(&cnt[levels - 1], lv0 + nb - levels);
+        }
     }
     __syncthreads();
     const int chunk = (levels + (int)blockDim.x - 1) / (int)blockDim.x;
     const int lo = min(levels, tid * chunk), hi = min(levels, lo + chunk);
-    // cnt[c] <- number of sequences with more than c blocks (inclusive suffix sum)
+    // cnt[c] <- entries at level c (inclusive prefix sum of the differences)
     int local = 0;
     for (int c = lo; c < hi; ++c) local += cnt[c];
-    int run = block_suffix_exclusive(local, warp_tot);
-    for (int c = hi - 1; c >= lo; --c) {
+    int run = block_prefix_exclusive(local, warp_tot);
+    for (int c = lo; c < hi; ++c) {
         run += cnt[c];
         cnt[c] = run;
     }
-    // start[c] <- entries of the levels above c (exclusive suffix sum of the new cnt)
+    __syncthreads();
+    // start[c] <- entries of the levels above c (exclusive suffix sum of the counts)
     local = 0;
     for (int c = lo; c < hi; ++c) local += cnt[c];
     int pos = block_suffix_exclusive(local, warp_tot);
@@ -192,9 +245,12 @@ __global__ void __launch_bounds__(1024) schedule_kernel(const int64_t* __restric
     for (int s = tid; s < n_seqs; s += blockDim.x) {
         int64_t q0, L, k0, Lk;
         seq_view(cu_seqlens, cu_seqlens_k, desc, s, q0, L, k0, Lk);
-        const int nb = min((int)((L + BQ - 1) / BQ), levels);
+        int nb, lv0;
+        seq_levels(L, Lk, causal, 0x7fffffff, nb, lv0);
+        lv0 = min(levels - 1, lv0 - base);
         for (int c = 0; c < nb; ++c) {
-            const int at = start[c] + atomicAdd(&cursor[c], 1);
+            const int lv = causal ? min(levels - 1, lv0 + c) : lv0;
+            const int at = start[lv] + atomicAdd(&cursor[lv], 1);
             items[at] = make_int4((int)q0, (int)L, c, (int)k0);  // (token counts are < 2^31)
             items_lk[at] = (int)Lk;
         }
@@ -968,8 +1024,8 @@ mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int
 
     const int levels = (int)(total_tokens / BQ) + 2;
     MOSAIC_CUDA_TRY(cudaMemsetAsync(workspace, 0, w.zero_bytes, s));
-    schedule_kernel<<<1, 1024, 0, s>>>(cu_seqlens, cu_seqlens_k, desc, n_seqs, levels, w.header,
-                                       w.cnt, w.start, w.cursor, w.items, w.items_lk);
+    schedule_kernel<<<1, 1024, 0, s>>>(cu_seqlens, cu_seqlens_k, desc, n_seqs, levels, causal ? 1 : 0,
+                                       w.header, w.cnt, w.start, w.cursor, w.items, w.items_lk);
     count_launch();
     MOSAIC_CUDA_TRY(cudaGetLastError());
 

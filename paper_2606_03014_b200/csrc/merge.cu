@@ -115,20 +115,37 @@ __global__ void __launch_bounds__(kMergeThreads) lse_merge_n_kernel(
     const int h = (int)(rowi - t * Hq);
     const int64_t o_stride = T * (int64_t)Hq * D, l_stride = (int64_t)Hq * T;
     const float* lrow = lse_parts + (int64_t)h * T + t;
-    float m = -INFINITY;
-    for (int p = 0; p < n_parts; ++p) m = fmaxf(m, lrow[p * l_stride]);
+    const __nv_bfloat16* orow = o_parts + rowi * D + c * 8;
+    // One pass, four parts in flight: running maximum m, weights relative to it, the accumulator
+    // rescaled when the maximum moves (an empty partial -- LSE = -inf -- has weight 0 and its O,
+    // which may be uninitialised, is multiplied by nothing).
+    float m = -INFINITY, z = 0.f;
     float acc[8];
 #pragma unroll
     for (int u = 0; u < 8; ++u) acc[u] = 0.f;
-    float z = 0.f;
-    if (m > -INFINITY) {
-        for (int p = 0; p < n_parts; ++p) {
-            const float l = lrow[p * l_stride];
-            if (l == -INFINITY) continue;  // an empty partial: weight 0, its O is not read
-            const float w = expf(l - m);
+    for (int p0 = 0; p0 < n_parts; p0 += 4) {
+        float l[4];
+        uint4 v[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const bool in = p0 + j < n_parts;
+            l[j] = in ? __ldg(lrow + (int64_t)(p0 + j) * l_stride) : -INFINITY;
+            v[j] = in ? __ldcs(reinterpret_cast<const uint4*>(orow + (int64_t)(p0 + j) * o_stride))
+                      : make_uint4(0u, 0u, 0u, 0u);
+        }
+        const float m_new = fmaxf(fmaxf(m, fmaxf(l[0], l[1])), fmaxf(l[2], l[3]));
+        if (m_new == -INFINITY) continue;
+        const float r = m == -INFINITY ? 0.f : expf(m - m_new);
+        z *= r;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) acc[u] *= r;
+        m = m_new;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (l[j] == -INFINITY) continue;
+            const float w = expf(l[j] - m);
             z += w;
-            const uint4 v = *reinterpret_cast<const uint4*>(o_parts + p * o_stride + rowi * D + c * 8);
-            const __nv_bfloat162* pv = reinterpret_cast<const __nv_bfloat162*>(&v);
+            const __nv_bfloat162* pv = reinterpret_cast<const __nv_bfloat162*>(&v[j]);
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const float2 f = __bfloat1622float2(pv[u]);
