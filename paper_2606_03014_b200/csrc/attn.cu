@@ -78,9 +78,11 @@ struct SchedHeader {
 
 struct Workspace {
     SchedHeader* header;
-    int* cnt;     // [levels]  sequences with exactly c+1 q blocks -> sequences with more than c
-    int* start;   // [levels]  first entry of level c (levels in descending order)
+    int* cnt;     // [levels]  sequences whose costliest block sits at the level
     int* cursor;  // [levels]
+    int* start;   // [levels]  sequences at higher levels (= the first rank of the level)
+    int* rank;    // [n_seqs]      rank of sequence s in descending cost order
+    int* first;   // [n_seqs + 1]  blocks of the sequences of lower rank (indexed by rank)
     int4* items;  // [capacity] (first q token of the sequence, its q length, q block, first k token)
     int* items_lk;  // [capacity] its k length
     size_t zero_bytes;  // prefix that must be zeroed before schedule_kernel
@@ -102,6 +104,10 @@ inline Workspace carve(void* base, int32_t n_seqs, int64_t total_tokens) {
     w.zero_bytes = off;
     w.start = reinterpret_cast<int*>(p + off);
     off += levels * sizeof(int);
+    w.rank = reinterpret_cast<int*>(p + off);
+    off += ((size_t)n_seqs + 1) * sizeof(int);
+    w.first = reinterpret_cast<int*>(p + off);
+    off += ((size_t)n_seqs + 2) * sizeof(int);
     off = (off + 15) & ~size_t(15);
     w.items = reinterpret_cast<int4*>(p + off);
     off += cap * sizeof(int4);
@@ -111,12 +117,17 @@ inline Workspace carve(void* base, int32_t n_seqs, int64_t total_tokens) {
     return w;
 }
 
-// Work items in descending cost order.  The cost of (sequence s, q block c) is the number of KV
-// tiles its rows visit: in 256-key units, level(s, c) = ceil(min(off_s + 256 (c + 1), Lk_s) / 256) - 1
-// with off_s = Lk_s - Lq_s when causal (the plain prefill: level = c), and ceil(Lk_s / 256) - 1 for
-// every block when not.  Counting sort over the levels, highest first; order inside a level is
-// arbitrary (the results do not depend on the schedule).  One block; the scans over the levels
-// are chunked over its threads.
+// A5, the length-sorted work list.  Sequences are ranked by the cost of their costliest q block --
+// level = ceil(visible keys / 256) of the LAST block, relative to the cheapest sequence of the batch:
+// for the plain prefill simply the length -- longest first (counting sort over the levels; order
+// inside a level is arbitrary, the results do not depend on the schedule), and a sequence's blocks
+// follow one another from the last (most KV tiles) to the first.  attn_fwd walks the list once per
+// KV head (KV head outermost, the q heads of its group innermost): the ~148 units in flight are then
+// neighbouring q blocks of ONE (sequence, KV head) -- they stream the same K / V, which stays in
+// L2 (16.8 MB for a 32 k-token head) -- instead of the same q block of every KV head (134 MB for a
+// 32 k-token sequence, more than the L2: round 1's order re-read K / V from DRAM 4.5-6x).  The
+// hand-out is dynamic, and the last units of the launch are the first blocks of the shortest
+// sequences, so the CTAs still finish together.  One block; the scans are chunked over its threads.
 
 // Sum of v over the threads with a larger thread index (whole block calls).
 __device__ __forceinline__ int block_suffix_exclusive(int v, int* warp_tot /* [32] shared */) {
@@ -171,86 +182,84 @@ __device__ __forceinline__ void seq_view(const int64_t* cu_q, const int64_t* cu_
     }
 }
 
-// The levels of a sequence's blocks: block c sits at level lv0 + (causal ? c : 0), clipped.
-__device__ __forceinline__ void seq_levels(int64_t L, int64_t Lk, int causal, int levels, int& nb,
-                                           int& lv0) {
-    nb = (int)((L + BQ - 1) / BQ);
-    if (causal) {
-        const int64_t off = Lk > L ? Lk - L : 0;
-        lv0 = (int)min((int64_t)levels - 1, off / BQ);  // level(c) = floor(off / 256) + c (+ a partial unit)
-    } else {
-        lv0 = (int)min((int64_t)levels - 1, Lk > 0 ? (Lk - 1) / BQ : 0);
-    }
+// Cost level of a sequence = that of its last q block: all its keys when causal (the last row sees
+// them all) or not, in 256-key units.
+__device__ __forceinline__ int seq_level(int64_t L, int64_t Lk) {
+    return (L > 0 && Lk > 0) ? (int)((Lk - 1) / BQ) : 0;
 }
 
 __global__ void __launch_bounds__(1024) schedule_kernel(const int64_t* __restrict__ cu_seqlens,
                                                         const int64_t* __restrict__ cu_seqlens_k,
                                                         const SeqDesc* __restrict__ desc,
-                                                        int n_seqs, int levels, int causal,
-                                                        SchedHeader* header, int* cnt, int* start,
-                                                        int* cursor, int4* items, int* items_lk) {
+                                                        int n_seqs, int levels, SchedHeader* header,
+                                                        int* cnt, int* start, int* cursor, int* rank,
+                                                        int* first, int4* items, int* items_lk) {
     __shared__ int warp_tot[32];
-    __shared__ int lv_min;  // levels are counted from the cheapest block of the batch: the arrays
+    __shared__ int lv_min;  // levels are counted from the cheapest sequence of the batch: the arrays
                             // hold total_q_tokens / 256 + 2 levels however long the keys are
+    __shared__ int carry;
     const int tid = threadIdx.x;
     if (tid == 0) lv_min = 0x7fffffff;
     __syncthreads();
     for (int s = tid; s < n_seqs; s += blockDim.x) {
         int64_t q0, L, k0, Lk;
         seq_view(cu_seqlens, cu_seqlens_k, desc, s, q0, L, k0, Lk);
-        int nb, lv0;
-        seq_levels(L, Lk, causal, 0x7fffffff, nb, lv0);
-        if (nb > 0) atomicMin(&lv_min, lv0);
+        if (L > 0) atomicMin(&lv_min, seq_level(L, Lk));
     }
     __syncthreads();
     const int base = lv_min == 0x7fffffff ? 0 : lv_min;
-    // cnt[] starts as a difference array: +w at the first level of a sequence's blocks, -w behind
-    // the last (causal: one block per level over nb levels; not causal: nb blocks at one level)
     for (int s = tid; s < n_seqs; s += blockDim.x) {
         int64_t q0, L, k0, Lk;
         seq_view(cu_seqlens, cu_seqlens_k, desc, s, q0, L, k0, Lk);
-        int nb, lv0;
-        seq_levels(L, Lk, causal, 0x7fffffff, nb, lv0);
-        lv0 = min(levels - 1, lv0 - base);
-        if (nb > 0) {
-            const int hi = causal ? min(levels, lv0 + nb) : lv0 + 1;  // (levels past the clip share the top one)
-            const int w = causal ? 1 : nb;
-            atomicAdd(&cnt[lv0], w);
-            if (hi < levels) atomicAdd(&cnt[hi], -w);
-            if (causal && lv0 + nb > levels) atomicAdd(&cnt[levels - 1], lv0 + nb - levels);
-        }
+        if (L > 0) atomicAdd(&cnt[min(levels - 1, seq_level(L, Lk) - base)], 1);
     }
     __syncthreads();
+    // start[c] <- sequences at the levels above c (exclusive suffix sum of the counts)
     const int chunk = (levels + (int)blockDim.x - 1) / (int)blockDim.x;
     const int lo = min(levels, tid * chunk), hi = min(levels, lo + chunk);
-    // cnt[c] <- entries at level c (inclusive prefix sum of the differences)
     int local = 0;
-    for (int c = lo; c < hi; ++c) local += cnt[c];
-    int run = block_prefix_exclusive(local, warp_tot);
-    for (int c = lo; c < hi; ++c) {
-        run += cnt[c];
-        cnt[c] = run;
-    }
-    __syncthreads();
-    // start[c] <- entries of the levels above c (exclusive suffix sum of the counts)
-    local = 0;
     for (int c = lo; c < hi; ++c) local += cnt[c];
     int pos = block_suffix_exclusive(local, warp_tot);
     for (int c = hi - 1; c >= lo; --c) {
         start[c] = pos;
         pos += cnt[c];
     }
-    if (tid == 0) header->n_items = pos;  // thread 0 owns level 0: pos = all entries
     __syncthreads();
+    // rank of every sequence (empty ones are not ranked), its block count by rank
+    const int n_ranked = start[0] + cnt[0];
     for (int s = tid; s < n_seqs; s += blockDim.x) {
         int64_t q0, L, k0, Lk;
         seq_view(cu_seqlens, cu_seqlens_k, desc, s, q0, L, k0, Lk);
-        int nb, lv0;
-        seq_levels(L, Lk, causal, 0x7fffffff, nb, lv0);
-        lv0 = min(levels - 1, lv0 - base);
+        int r = -1;
+        if (L > 0) {
+            const int lv = min(levels - 1, seq_level(L, Lk) - base);
+            r = start[lv] + atomicAdd(&cursor[lv], 1);
+            first[r] = (int)((L + BQ - 1) / BQ);
+        }
+        rank[s] = r;
+    }
+    if (tid == 0) carry = 0;
+    __syncthreads();
+    // first[r] <- blocks of the sequences of lower rank (exclusive prefix sum, 1024 ranks a round)
+    for (int r0 = 0; r0 < n_ranked; r0 += (int)blockDim.x) {
+        const int r = r0 + tid;
+        const int nb = r < n_ranked ? first[r] : 0;
+        const int before = carry + block_prefix_exclusive(nb, warp_tot);
+        if (r < n_ranked) first[r] = before;
+        __syncthreads();
+        if (tid == (int)blockDim.x - 1) carry = before + nb;
+        __syncthreads();
+    }
+    if (tid == 0) header->n_items = carry;
+    for (int s = tid; s < n_seqs; s += blockDim.x) {
+        const int r = rank[s];
+        if (r < 0) continue;
+        int64_t q0, L, k0, Lk;
+        seq_view(cu_seqlens, cu_seqlens_k, desc, s, q0, L, k0, Lk);
+        const int nb = (int)((L + BQ - 1) / BQ);
+        const int at0 = first[r];
         for (int c = 0; c < nb; ++c) {
-            const int lv = causal ? min(levels - 1, lv0 + c) : lv0;
-            const int at = start[lv] + atomicAdd(&cursor[lv], 1);
+            const int at = at0 + (nb - 1 - c);  // the last block (most KV tiles) first
             items[at] = make_int4((int)q0, (int)L, c, (int)k0);  // (token counts are < 2^31)
             items_lk[at] = (int)Lk;
         }
@@ -269,6 +278,7 @@ struct AttnParams {
     int Hq, Hkv;
     float scale_log2;  // |softmax_scale| * log2(e); a negative scale negates Q inside the MMA
     float inv_group;   // 1 / (Hq / Hkv)
+    int group;         // Hq / Hkv
     int causal;        // 0: every q row sees all the keys of its sequence
     int o_align32;     // o is 32-byte aligned: the epilogue may use 256-bit stores
 };
@@ -406,7 +416,8 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
     const uint32_t mma_lock = bars + 8 * kNumBars + 4;  // the two issuers take turns (see below)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int n_work = p.header->n_items * p.Hq;
+    const int n_items = p.header->n_items;
+    const int n_work = n_items * p.Hq;
 
     if (tid == 0) {
         ptx::prefetch_tensormap(&tm_q);
@@ -540,8 +551,11 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                 w = __shfl_sync(0xffffffffu, w, 0);
                 f_h = -1;
                 if (w < n_work) {
-                    const int item = w / p.Hq;
-                    f_h = w - item * p.Hq;
+                    // unit w = (KV head g, work-list entry, q head r of g's group), r fastest
+                    const int per_g = n_items * p.group;
+                    const int g = w / per_g, rem = w - g * per_g;
+                    const int item = rem / p.group;
+                    f_h = g * p.group + (rem - item * p.group);
                     f_it = __ldg(p.items + item);
                     f_lk = __ldg(p.items_lk + item);
                 }
@@ -1024,8 +1038,8 @@ mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int
 
     const int levels = (int)(total_tokens / BQ) + 2;
     MOSAIC_CUDA_TRY(cudaMemsetAsync(workspace, 0, w.zero_bytes, s));
-    schedule_kernel<<<1, 1024, 0, s>>>(cu_seqlens, cu_seqlens_k, desc, n_seqs, levels, causal ? 1 : 0,
-                                       w.header, w.cnt, w.start, w.cursor, w.items, w.items_lk);
+    schedule_kernel<<<1, 1024, 0, s>>>(cu_seqlens, cu_seqlens_k, desc, n_seqs, levels, w.header, w.cnt,
+                                       w.start, w.cursor, w.rank, w.first, w.items, w.items_lk);
     count_launch();
     MOSAIC_CUDA_TRY(cudaGetLastError());
 
@@ -1041,6 +1055,7 @@ mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int
     p.Hkv = Hkv;
     p.scale_log2 = fabsf(softmax_scale) * kLog2e;
     p.inv_group = 1.0f / (float)(Hq / Hkv);
+    p.group = Hq / Hkv;
     p.causal = causal ? 1 : 0;
     p.o_align32 = (reinterpret_cast<uintptr_t>(o) & 31u) == 0 ? 1 : 0;
     const int negate_q = softmax_scale < 0.f ? 1 : 0;
