@@ -154,8 +154,13 @@ def test_identical_keys_prefix_mean_every_row():
 
 
 def _config_batch(cfg, seed):
+    """The survivors' batch as bench.py forms it: the vote-fraction gate on configs[1..3], the
+    weighted-confidence gate on configs[4] (the headline step), first max_attn_seqs survivors."""
     gi = wl.gate_inputs(cfg, seed)
-    og = oracle.gate(gi.answers, gi.tau)
+    if cfg.config_id == 5:
+        og = oracle.gate(gi.answers, gi.tau, gi.expert_conf, 1)
+    else:
+        og = oracle.gate(gi.answers, gi.tau)
     oc = oracle.compact(og["bypass"], gi.ctx_len)
     n = oc["n_survivors"] if cfg.max_attn_seqs is None else min(cfg.max_attn_seqs, oc["n_survivors"])
     return oc["cu_seqlens"][:n + 1]
@@ -193,6 +198,17 @@ def test_configs_sampled_rows_and_structured(cid, n_random):
     del q, k, v, o, lse
     torch.cuda.empty_cache()
     eo, el = _identical_keys_check(np.diff(cu).tolist(), cfg.Hq, cfg.Hkv, cfg.D, seed=cid)
+    assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
+
+
+def test_thousands_of_short_sequences_full():
+    """More sequences than the scheduling kernel has threads (its ranking and prefix sums run in
+    rounds of 1024) and far more work units than CTAs, lengths 1..300 with empty ones in between:
+    every row against the oracle."""
+    g = np.random.default_rng(77)
+    lengths = g.integers(0, 301, size=2600).tolist()
+    lengths[0], lengths[1], lengths[-1] = 300, 0, 257
+    eo, el = _full_case(lengths, 2, 1, 64, seed=29)
     assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
 
 
