@@ -37,7 +37,7 @@ sys.path.insert(0, str(ROOT))
 METRIC = "gated agg-prefill attn TFLOP/s"
 UNIT = "TFLOP/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
-TRAFFIC_SOURCE = "profiles/traffic.json (ncu --set full, static: not measured in this run)"
+TRAFFIC_SOURCE = "profiles/traffic.json (ncu, static)"
 ALL_LEGS = ("gate", "q24", "lse_merge", "lse_merge_n", "rope", "assemble", "decode", "attn_kv",
             "prefix", "chunked", "per_config", "gated_stage", "e2e", "cpu")
 
@@ -266,8 +266,11 @@ def timed(torch, fn, n, warm=2):
 
 def hbm_leg(ms, byts, pk, traffic=None):
     t = float(np.median(ms)) * 1e-3
-    return {"us": r3(t * 1e6), "us_best": r3(float(ms.min()) * 1e3), "gbs": r3(byts / t / 1e9),
-            "frac": r3(byts / t / 1e9 / pk["hbm_gbs"]), "bytes": int(byts), "traffic": traffic}
+    leg = {"us": r3(t * 1e6), "us_best": r3(float(ms.min()) * 1e3), "gbs": r3(byts / t / 1e9),
+           "frac": r3(byts / t / 1e9 / pk["hbm_gbs"]), "bytes": int(byts)}
+    if traffic is not None:
+        leg["traffic"] = traffic
+    return leg
 
 
 def tensor_leg(ms, fl, pk):
@@ -772,8 +775,7 @@ def run_product(args):
                      "traffic": static_traffic("attn_fwd_c5_dram_bytes_per_launch"),
                      "traffic_source": TRAFFIC_SOURCE, "kernel": "attn_fwd<128> (+ schedule_kernel)",
                      "ms_per_launch": r3(attn_t * 1e3),
-                     "peak_kind": ("sustained" if sustained else "burst") + " bf16_tflops: the timed "
-                                  "region is %.1f s" % secs_max,
+                     "peak_kind": ("sustained" if sustained else "burst") + " (timed region %.1f s)" % secs_max,
                      "frac_burst": r3(attn_tflops / pk["bf16_tflops"]),
                      "frac_nominal_2250": r3(attn_tflops / 2250.0)},
         "gate": gate_info,
