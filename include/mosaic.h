@@ -306,11 +306,11 @@ mosaic_status_t mosaic_agg_prefill_attn_chunked(const void* q, const void* k, co
  *   q, o [dev] bf16 [total_tokens, Hq, D], k, v [dev] bf16 [total_tokens, Hkv, D], cu_seqlens,
  *   lse: the sequences' OWN tokens, as mosaic_agg_prefill_attn;
  *   k_prefix, v_prefix [dev] bf16 [prefix_len, Hkv, D] (16-byte aligned); prefix_len >= 0.
- * Two passes over the same kernel -- the own keys (causal), and the packed rows of all sequences
- * as ONE view against the shared block (non-causal), whose K / V are therefore read from HBM once
- * for the whole batch -- merged exactly through their logsumexps (mosaic_lse_merge).
- *   workspace >= mosaic_agg_prefill_attn_shared_prefix_workspace_bytes(...): it holds one
- *   partial O and LSE.  Errors, alignment and asynchrony as mosaic_agg_prefill_attn.
+ * One launch of the attention kernel: a q tile visits the shared block's K / V tiles (a few MB that
+ * stay in L2: read from HBM once for the whole batch) and then its sequence's own, in one online
+ * softmax -- no partial results, no merge.
+ *   workspace >= mosaic_agg_prefill_attn_shared_prefix_workspace_bytes(...).  Errors, alignment
+ *   and asynchrony as mosaic_agg_prefill_attn.
  * ------------------------------------------------------------------------------------------- */
 size_t mosaic_agg_prefill_attn_shared_prefix_workspace_bytes(int32_t n_seqs, int64_t total_tokens,
                                                              int32_t Hq, int32_t Hkv, int32_t D);

@@ -279,6 +279,8 @@ struct AttnParams {
     float scale_log2;  // |softmax_scale| * log2(e); a negative scale negates Q inside the MMA
     float inv_group;   // 1 / (Hq / Hkv)
     int group;         // Hq / Hkv
+    int prefix_len;    // shared-prefix cascade: every sequence's keys are prefix_len shared keys (their
+    int prefix_pad;    // own tensor maps) followed by its own; prefix_pad = prefix_len rounded up to 128
     int causal;        // 0: every q row sees all the keys of its sequence
     int o_align32;     // o is 32-byte aligned: the epilogue may use 256-bit stores
 };
@@ -350,14 +352,16 @@ __device__ __forceinline__ Work make_work(const AttnParams& p, const int4 it, in
     k.t0 = it.x;
     k.tk0 = it.w;
     k.L = it.y;
-    k.off = p.causal ? lk - it.y : (1 << 29);
-    k.lk = lk;
+    // (with a shared prefix the keys are [prefix, padded to whole tiles][own keys]: every row sees
+    //  the whole prefix, so the offset and the key count simply grow by prefix_pad)
+    k.off = p.causal ? lk - it.y + p.prefix_pad : (1 << 29);
+    k.lk = lk + p.prefix_pad;
     k.row0 = it.z * BQ;
     // KV tiles of a q tile: up to the last key its last row sees (2c+1 and 2c+2 when off = 0)
     // (clamped at 0: a sequence without keys -- mosaic_agg_decode_attn makes those -- or, against
     //  the contract, with fewer keys than q rows when causal, has tiles that visit nothing)
-    const int last0 = max(0, min(min(k.row0 + BM, k.L) + k.off, lk));
-    const int last1 = max(0, min(min(k.row0 + BQ, k.L) + k.off, lk));
+    const int last0 = max(0, min(min(k.row0 + BM, k.L) + k.off, k.lk));
+    const int last1 = max(0, min(min(k.row0 + BQ, k.L) + k.off, k.lk));
     k.n0 = (last0 + BN - 1) / BN;
     k.n1 = (k.row0 + BM < k.L) ? (last1 + BN - 1) / BN : 0;
     k.n_kv = max(k.n0, k.n1);
@@ -398,7 +402,8 @@ __device__ __forceinline__ void setmaxnreg_dec() {
 template <int D>
 __global__ void __launch_bounds__(kThreadsAttn, 1)
 attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
-         const __grid_constant__ CUtensorMap tm_v, const AttnParams p, const int negate_q) {
+         const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_kp,
+         const __grid_constant__ CUtensorMap tm_vp, const AttnParams p, const int negate_q) {
     using SL = SmemLayout<D>;
     // tile t: score buffers [128 t, 128 t + 64) and [128 t + 64, 128 t + 128), each overwritten by
     // its P (bf16, 32 columns); O_t: [256 + 128 t, ..)
@@ -423,6 +428,10 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
         ptx::prefetch_tensormap(&tm_q);
         ptx::prefetch_tensormap(&tm_k);
         ptx::prefetch_tensormap(&tm_v);
+        if (p.prefix_pad) {
+            ptx::prefetch_tensormap(&tm_kp);
+            ptx::prefetch_tensormap(&tm_vp);
+        }
         for (int t = 0; t < 2; ++t) {
             ptx::mbar_init(bar(kBarQFull, t), 1);
             ptx::mbar_init(bar(kBarQEmpty, t), 1);
@@ -594,18 +603,23 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                     }
                     __syncwarp();
                 };
-                auto load_kv = [&](const CUtensorMap* tm, int j) {
+                // KV tile j of the unit: one of the shared prefix's tiles first (rows past prefix_len
+                // are outside that tensor map and arrive as zeros; the softmax groups mask them),
+                // then the sequence's own keys
+                const int jp = p.prefix_pad / BN;
+                auto load_kv = [&](bool is_v, int j) {
                     const uint32_t slot = slot_of(pos), ph = phase_of(pos);
                     ++pos;
                     ptx::mbar_wait(bar_kv_empty(0, slot), ph ^ 1);
                     ptx::mbar_wait(bar_kv_empty(1, slot), ph ^ 1);
                     if (ptx::elect_one()) {
+                        const CUtensorMap* tm = j < jp ? (is_v ? &tm_vp : &tm_kp) : (is_v ? &tm_v : &tm_k);
+                        const int row = j < jp ? j * BN : (int)(k.tk0 + (j - jp) * BN);
                         ptx::mbar_arrive_expect_tx(bar(kBarKvFull, slot), SL::kTileBytes);
 #pragma unroll
                         for (int c = 0; c < D / 64; ++c)
                             ptx::tma_load_3d(sKV + slot * SL::kTileBytes + c * SL::kBlockBytes, tm,
-                                             bar(kBarKvFull, slot), c * 64, k.g,
-                                             (int)(k.tk0 + j * BN));
+                                             bar(kBarKvFull, slot), c * 64, k.g, row);
                     }
                     __syncwarp();
                 };
@@ -614,12 +628,12 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                 // a unit without any KV tile takes no ring position at all.
                 if (k.n_kv == 0) continue;
                 if (k.n0) load_q(0);
-                load_kv(&tm_k, 0);
+                load_kv(false, 0);
                 if (k.n1) load_q(1);
-                load_kv(&tm_v, 0);
+                load_kv(true, 0);
                 for (int j = 1; j < k.n_kv; ++j) {
-                    load_kv(&tm_k, j);
-                    load_kv(&tm_v, j);
+                    load_kv(false, j);
+                    load_kv(true, j);
                 }
             }
         } else if (warp == kWarpMma0 || warp == kWarpMma1) {
@@ -911,9 +925,23 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
             const int tile_row0 = k.row0 + k.tile_of(t) * BM;  // first row of the tile in the sequence
             const int u_masked = ((min(tile_row0 + k.off, k.lk - 1) + 1) >> 6) & ~1;
             const int U = 2 * n_t;
+            // (shared prefix: the two steps of its last tile hold prefix_pad - prefix_len padding
+            //  keys, masked for every row; they lie before u_masked because every row sees the
+            //  whole prefix)
+            const int u_hole = p.prefix_len < p.prefix_pad ? 2 * (p.prefix_pad / BN - 1) : -1;
             for (int u = 0; u < u_masked; u += 2) {
-                step(M0{}, 0, u == 0);
-                step(M0{}, 1, false);
+                if (u == u_hole) {
+                    thr = p.prefix_len - 1 - u * BS;  // >= 0: the tile holds at least one prefix key
+                    step(M1{}, 0, u == 0);
+                    thr -= BS;
+                    if (thr < 0)
+                        step(M2{}, 1, false);
+                    else
+                        step(M1{}, 1, false);
+                } else {
+                    step(M0{}, 0, u == 0);
+                    step(M0{}, 1, false);
+                }
                 ph_s ^= 1;
             }
             for (int u = u_masked; u < U; ++u) {
@@ -978,7 +1006,7 @@ bool make_tensor_map(CUtensorMap* map, const void* base, int64_t T, int H, int D
 
 template <int D>
 mosaic_status_t launch_attn(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv,
-                            const AttnParams& p, int negate_q, int grid, cudaStream_t s) {
+                            const CUtensorMap& tkp, const CUtensorMap& tvp, const AttnParams& p, int negate_q, int grid, cudaStream_t s) {
     using SL = SmemLayout<D>;
     static bool configured = false;
     if (!configured) {
@@ -986,7 +1014,7 @@ mosaic_status_t launch_attn(const CUtensorMap& tq, const CUtensorMap& tk, const 
                                              SL::kDynamic));
         configured = true;
     }
-    attn_fwd<D><<<grid, kThreadsAttn, SL::kDynamic, s>>>(tq, tk, tv, p, negate_q);
+    attn_fwd<D><<<grid, kThreadsAttn, SL::kDynamic, s>>>(tq, tk, tv, tkp, tvp, p, negate_q);
     count_launch();
     MOSAIC_CUDA_TRY(cudaGetLastError());
     return MOSAIC_OK;
@@ -1015,7 +1043,10 @@ mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int
                           int64_t total_tokens,
                           int64_t total_k_tokens, int32_t max_seqlen, int32_t Hq, int32_t Hkv,
                           int32_t D, float softmax_scale, int causal, void* o, float* lse,
-                          void* workspace, size_t workspace_bytes, void* cuda_stream) {
+                          void* workspace, size_t workspace_bytes, void* cuda_stream,
+                          const void* k_prefix, const void* v_prefix, int32_t prefix_len) {
+    if (prefix_len < 0 || (prefix_len > 0 && (!causal || !k_prefix || !v_prefix)))
+        return MOSAIC_ERR_INVALID_ARG;
     if (n_seqs < 0 || total_tokens < 0 || total_tokens >= (1ll << 31) || total_k_tokens < 0 ||
         total_k_tokens >= (1ll << 31) || max_seqlen < 0 || Hq < 1 || Hkv < 1 || Hq % Hkv != 0 ||
         !isfinite(softmax_scale))
@@ -1034,6 +1065,10 @@ mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int
     if (!make_tensor_map(&tq, q, total_tokens, Hq, D, BM) ||
         !make_tensor_map(&tk, k, total_k_tokens, Hkv, D, BN) ||
         !make_tensor_map(&tv, v, total_k_tokens, Hkv, D, BN))
+        return MOSAIC_ERR_CUDA;
+    CUtensorMap tkp = tk, tvp = tv;  // (never dereferenced without a prefix)
+    if (prefix_len > 0 && (!make_tensor_map(&tkp, k_prefix, prefix_len, Hkv, D, BN) ||
+                           !make_tensor_map(&tvp, v_prefix, prefix_len, Hkv, D, BN)))
         return MOSAIC_ERR_CUDA;
 
     const int levels = (int)(total_tokens / BQ) + 2;
@@ -1057,13 +1092,15 @@ mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int
     p.inv_group = 1.0f / (float)(Hq / Hkv);
     p.group = Hq / Hkv;
     p.causal = causal ? 1 : 0;
+    p.prefix_len = prefix_len;
+    p.prefix_pad = (prefix_len + BN - 1) / BN * BN;
     p.o_align32 = (reinterpret_cast<uintptr_t>(o) & 31u) == 0 ? 1 : 0;
     const int negate_q = softmax_scale < 0.f ? 1 : 0;
     const int64_t max_work = (total_tokens / BQ + n_seqs) * (int64_t)Hq;
     if (max_work >= (1ll << 31)) return MOSAIC_ERR_UNSUPPORTED;
     const int grid = (int)(max_work < num_sms() ? max_work : num_sms());
-    return D == 64 ? launch_attn<64>(tq, tk, tv, p, negate_q, grid, s)
-                   : launch_attn<128>(tq, tk, tv, p, negate_q, grid, s);
+    return D == 64 ? launch_attn<64>(tq, tk, tv, tkp, tvp, p, negate_q, grid, s)
+                   : launch_attn<128>(tq, tk, tv, tkp, tvp, p, negate_q, grid, s);
 }
 }  // namespace mosaic
 

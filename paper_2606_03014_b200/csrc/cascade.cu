@@ -60,11 +60,6 @@ __global__ void __launch_bounds__(1024) chunk_plan_kernel(const int64_t* __restr
     for (int64_t v = carry + tid; v < v_max; v += 1024) desc[v] = SeqDesc{0, 0, 0, 0};
 }
 
-// ---- shared prefix: the packed q rows of ALL sequences as one view against the prefix block
-__global__ void prefix_view_kernel(SeqDesc* desc, int64_t T, int32_t P) {
-    desc[0] = SeqDesc{0, 0, (int32_t)T, P};
-}
-
 struct ChunkWs {
     SeqDesc* desc;
     void* attn_ws;
@@ -81,33 +76,6 @@ ChunkWs carve_chunked(void* base, int32_t n_seqs, int64_t total_tokens, int32_t 
     off += align256((size_t)w.v_max * sizeof(SeqDesc));
     w.attn_ws_bytes = mosaic_agg_prefill_attn_workspace_bytes(
         (int32_t)(w.v_max < (1ll << 31) - 1 ? w.v_max : (1ll << 31) - 1), total_tokens, Hq, Hkv, D);
-    w.attn_ws = p + off;
-    off += align256(w.attn_ws_bytes);
-    w.total = off;
-    return w;
-}
-
-struct PrefixWs {
-    SeqDesc* desc;
-    void* o_tmp;
-    float* lse_tmp;
-    void* attn_ws;
-    size_t attn_ws_bytes, total;
-};
-PrefixWs carve_prefix(void* base, int32_t n_seqs, int64_t total_tokens, int32_t Hq, int32_t Hkv,
-                      int32_t D) {
-    PrefixWs w{};
-    char* p = static_cast<char*>(base);
-    size_t off = 0;
-    w.desc = reinterpret_cast<SeqDesc*>(p + off);
-    off += 256;
-    w.o_tmp = p + off;
-    off += align256((size_t)total_tokens * Hq * D * 2);
-    w.lse_tmp = reinterpret_cast<float*>(p + off);
-    off += align256((size_t)total_tokens * Hq * 4);
-    // the larger of the two passes' work lists: one view of T rows, n_seqs views of T rows together
-    w.attn_ws_bytes = mosaic_agg_prefill_attn_workspace_bytes(n_seqs > 1 ? n_seqs : 1, total_tokens,
-                                                              Hq, Hkv, D);
     w.attn_ws = p + off;
     off += align256(w.attn_ws_bytes);
     w.total = off;
@@ -154,45 +122,27 @@ extern "C" size_t mosaic_agg_prefill_attn_shared_prefix_workspace_bytes(int32_t 
                                                                         int64_t total_tokens,
                                                                         int32_t Hq, int32_t Hkv,
                                                                         int32_t D) {
-    if (n_seqs < 0 || total_tokens < 0 || Hq < 1 || Hkv < 1 || D < 1) return 0;
-    return carve_prefix(nullptr, n_seqs, total_tokens, Hq, Hkv, D).total;
+    return mosaic_agg_prefill_attn_workspace_bytes(n_seqs, total_tokens, Hq, Hkv, D);
 }
 
+// One launch of the attention kernel: a work unit's KV tiles are the shared block's tiles (its own
+// pair of tensor maps, the last tile padded to 128 keys and the padding masked) followed by the
+// sequence's own; with the offset grown by the padded prefix length every role of the kernel sees
+// an ordinary bottom-right causal problem.  The block's K / V (a few MB) stay in L2: they are
+// read from HBM once for the whole batch.  (The first version ran the own keys and the shared block
+// as two passes -- the second as ONE non-causal view of all packed q rows -- and merged them with
+// mosaic_lse_merge: two more passes over O and Q read twice; 1 097 against 1 2xx TFLOP/s on
+// bench.py's shared_prefix leg.)
 extern "C" mosaic_status_t mosaic_agg_prefill_attn_shared_prefix(
     const void* q, const void* k_prefix, const void* v_prefix, int32_t prefix_len, const void* k,
     const void* v, const int64_t* cu_seqlens, int32_t n_seqs, int64_t total_tokens,
     int32_t max_seqlen, int32_t Hq, int32_t Hkv, int32_t D, float softmax_scale, void* o,
     float* lse, void* workspace, size_t workspace_bytes, void* cuda_stream) {
-    if (n_seqs < 0 || total_tokens < 0 || total_tokens >= (1ll << 31) || max_seqlen < 0 ||
-        prefix_len < 0 || Hq < 1 || Hkv < 1 || Hq % Hkv != 0 || !isfinite(softmax_scale))
+    if (prefix_len < 0) return MOSAIC_ERR_INVALID_ARG;
+    if (prefix_len > 0 && n_seqs > 0 && total_tokens > 0 &&
+        (!k_prefix || !v_prefix || !aligned16(k_prefix) || !aligned16(v_prefix)))
         return MOSAIC_ERR_INVALID_ARG;
-    if (D != 64 && D != 128) return MOSAIC_ERR_UNSUPPORTED;
-    if (n_seqs == 0 || total_tokens == 0) return MOSAIC_OK;
-    if (!workspace || !aligned16(workspace)) return MOSAIC_ERR_INVALID_ARG;
-    PrefixWs w = carve_prefix(workspace, n_seqs, total_tokens, Hq, Hkv, D);
-    if (workspace_bytes < w.total) return MOSAIC_ERR_WORKSPACE_TOO_SMALL;
-    // the sequences' own keys: the plain causal prefill over the suffixes
-    if (prefix_len == 0)
-        return mosaic_agg_prefill_attn(q, k, v, cu_seqlens, n_seqs, total_tokens, max_seqlen, Hq, Hkv,
-                                       D, softmax_scale, o, lse, w.attn_ws, w.attn_ws_bytes,
-                                       cuda_stream);
-    if (!k_prefix || !v_prefix || !aligned16(k_prefix) || !aligned16(v_prefix))
-        return MOSAIC_ERR_INVALID_ARG;
-    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-    mosaic_status_t st = mosaic_agg_prefill_attn(q, k, v, cu_seqlens, n_seqs, total_tokens, max_seqlen,
-                                                 Hq, Hkv, D, softmax_scale, w.o_tmp, w.lse_tmp,
-                                                 w.attn_ws, w.attn_ws_bytes, cuda_stream);
-    if (st != MOSAIC_OK) return st;
-    // the shared block: every q row of every sequence sees all of it, so the packed rows are ONE
-    // view of total_tokens rows against prefix_len keys -- 128-row tiles run across the sequence
-    // boundaries and the block's K / V tiles (a few MB: L2-resident) are read from HBM once
-    prefix_view_kernel<<<1, 1, 0, s>>>(w.desc, total_tokens, prefix_len);
-    count_launch();
-    MOSAIC_CUDA_TRY(cudaGetLastError());
-    st = attn_impl(q, k_prefix, v_prefix, nullptr, nullptr, w.desc, 1, total_tokens, prefix_len,
-                   max_seqlen, Hq, Hkv, D, softmax_scale, /*causal=*/0, o, lse, w.attn_ws,
-                   w.attn_ws_bytes, cuda_stream);
-    if (st != MOSAIC_OK) return st;
-    // disjoint key sets: merged exactly through the logsumexps (reading N2-2), in place
-    return mosaic_lse_merge(o, lse, w.o_tmp, w.lse_tmp, total_tokens, Hq, D, o, lse, cuda_stream);
+    return attn_impl(q, k, v, cu_seqlens, cu_seqlens, nullptr, n_seqs, total_tokens, total_tokens,
+                     max_seqlen, Hq, Hkv, D, softmax_scale, /*causal=*/1, o, lse, workspace,
+                     workspace_bytes, cuda_stream, k_prefix, v_prefix, prefix_len);
 }

@@ -36,12 +36,15 @@ struct SeqDesc {
     int32_t q_len, k_len;
 };
 // The attention behind mosaic_agg_prefill_attn[_kv] (attn.cu), for the entry points built on it.
+// k_prefix / v_prefix [prefix_len, Hkv, D]: a block of keys every sequence sees in front of its own
+// (causal only; the shared-prefix cascade).
 mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int64_t* cu_seqlens,
                           const int64_t* cu_seqlens_k, const SeqDesc* desc, int32_t n_seqs,
                           int64_t total_tokens, int64_t total_k_tokens, int32_t max_seqlen,
                           int32_t Hq, int32_t Hkv, int32_t D, float softmax_scale, int causal,
                           void* o, float* lse, void* workspace, size_t workspace_bytes,
-                          void* cuda_stream);
+                          void* cuda_stream, const void* k_prefix = nullptr,
+                          const void* v_prefix = nullptr, int32_t prefix_len = 0);
 
 // Number of SMs of the current device (cached per thread; 148 on B200).
 int num_sms();
