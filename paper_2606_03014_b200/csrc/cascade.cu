@@ -4,8 +4,7 @@
 //   mosaic_agg_prefill_attn_shared_prefix  shared-prefix cascade: every survivor's context starts
 //                                          with the same block of keys (the aggregator's prompt
 //                                          template, P:L225 / P:L377 `Aggregator(q, {a_i})`)
-// Only plans, descriptors and the order of calls live here; the attention is attn.cu's kernel and
-// the merge is merge.cu's.
+// Only plans and descriptors live here; the attention is attn.cu's kernel.
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
@@ -131,7 +130,7 @@ extern "C" size_t mosaic_agg_prefill_attn_shared_prefix_workspace_bytes(int32_t 
 // an ordinary bottom-right causal problem.  The block's K / V (a few MB) stay in L2: they are
 // read from HBM once for the whole batch.  (The first version ran the own keys and the shared block
 // as two passes -- the second as ONE non-causal view of all packed q rows -- and merged them with
-// mosaic_lse_merge: two more passes over O and Q read twice; 1 097 against 1 2xx TFLOP/s on
+// mosaic_lse_merge: two more passes over O and Q read twice; 1 097 against 1 177 TFLOP/s on
 // bench.py's shared_prefix leg.)
 extern "C" mosaic_status_t mosaic_agg_prefill_attn_shared_prefix(
     const void* q, const void* k_prefix, const void* v_prefix, int32_t prefix_len, const void* k,
