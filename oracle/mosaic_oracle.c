@@ -20,6 +20,13 @@
  *                     (P:L188 only licenses a substitute estimator) -- PARITY UNPINNED by the
  *                     paper; pinned only by reductions (equal weights == vote fraction,
  *                     unanimous == 1, all-distinct == w_mode/sum w) and exact rationals.
+ *   oracle_gate_ext (abstention sentinel, weighted argmax, tau per question): the
+ *                     paper defines none of them (P:L188, L251, L367 only name the openings) --
+ *                     PARITY UNPINNED by the paper; pinned to DESIGN.md readings N3-1..N3-3 by
+ *                     hand-worked k = 3 cases under both abstention policies, reduction to
+ *                     oracle_gate when no sentinel occurs, an always-abstaining extra expert that
+ *                     must drop out, equal weights == count plurality, exact rationals
+ *                     (tests/test_oracle_gate_ext.py).
  *   oracle_compact  : numpy.flatnonzero / numpy.cumsum special case, S = Q - sum(bypass),
  *                     all-bypass / none-bypass cases.
  *   oracle_attn_*   : L=1 returns V; identical keys give causal prefix mean and
