@@ -728,30 +728,34 @@ def run_product(args):
     if gate_info is not None and "q24" in legs:
         gate_info["q24"] = bench_gate_q24(torch, mosaic, pk)
     nxt = {}
-    if "lse_merge" in legs:
-        nxt["lse_merge"] = bench_lse_merge(torch, mosaic, pk, C2T, C2.Hq, C2.D)
-    if "lse_merge_n" in legs:
-        nxt["lse_merge_n"] = bench_lse_merge_n(torch, mosaic, pk, C2T, C2.Hq, C2.D)
-    if "rope" in legs:
-        nxt["rope"] = bench_rope(torch, mosaic, pk, C2T, C2.Hq, C2.Hkv, C2.D)
-    if "assemble" in legs:
-        nxt["assemble"] = bench_assemble(torch, mosaic, pk)
-    if "decode" in legs:
-        nxt["decode"] = bench_decode(torch, mosaic, pk)
-    if "attn_kv" in legs:
-        nxt["attn_kv"] = bench_attn_kv(torch, mosaic, pk)
-    if "prefix" in legs:
-        nxt["shared_prefix"] = bench_prefix(torch, mosaic, pk)
-    if "chunked" in legs:
-        nxt["chunked"] = bench_chunked(torch, mosaic, pk)
+
+    def leg(name, key, fn):
+        """A supplementary leg: a failure is recorded in the line, loudly, and does
+        not take the headline measurements down with it."""
+        if name not in legs:
+            return
+        try:
+            nxt[key] = fn()
+        except Exception as e:  # noqa: BLE001
+            print(f"bench.py: leg {key} failed: {e!r}", file=sys.stderr, flush=True)
+            nxt[key] = {"error": repr(e)[:120]}
+            torch.cuda.empty_cache()
+
+    leg("lse_merge", "lse_merge", lambda: bench_lse_merge(torch, mosaic, pk, C2T, C2.Hq, C2.D))
+    leg("lse_merge_n", "lse_merge_n", lambda: bench_lse_merge_n(torch, mosaic, pk, C2T, C2.Hq, C2.D))
+    leg("rope", "rope", lambda: bench_rope(torch, mosaic, pk, C2T, C2.Hq, C2.Hkv, C2.D))
+    leg("assemble", "assemble", lambda: bench_assemble(torch, mosaic, pk))
+    leg("decode", "decode", lambda: bench_decode(torch, mosaic, pk))
+    leg("attn_kv", "attn_kv", lambda: bench_attn_kv(torch, mosaic, pk))
+    leg("prefix", "shared_prefix", lambda: bench_prefix(torch, mosaic, pk))
+    leg("chunked", "chunked", lambda: bench_chunked(torch, mosaic, pk))
     per_config = bench_per_config(torch, mosaic, wl, pk) if "per_config" in legs else {}
     attn_t = float(np.median(attn_ms)) * 1e-3
     attn_tflops = flops / attn_t / 1e12
     c5 = tensor_leg(attn_ms, flops, pk)
     c5.update(seqs=S, tokens=T)
     per_config["C5"] = c5
-    if "gated_stage" in legs:
-        nxt["gated_stage"] = bench_gated_stage(torch, mosaic, wl)
+    leg("gated_stage", "gated_stage", lambda: bench_gated_stage(torch, mosaic, wl))
     cpu = None
     if "cpu" in legs:
         f, t, threads, desc = oracle_sample(cfg, 0, args.cpu_rows)
