@@ -281,3 +281,34 @@ def test_stage_host_chunked_matches_oracle():
     lse = r["lse"][:cfg.Hq * T].view(cfg.Hq, T)
     eo, el = P.check_attn_rows(o, lse, q, k, v, cu, rs, rh, rp, scale)
     assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
+
+
+def test_stage_host_weighted_gate_and_first_survivors_only():
+    """mosaic_stage_host as bench.py's end-to-end leg calls it: the weighted-confidence gate and
+    attention over the first max_attn_seqs survivors only (configs[1] inputs, 10 sequences)."""
+    from paper_2606_03014_b200 import mosaic
+    cfg = wl.C2
+    gi = wl.gate_inputs(cfg, 2)
+    want = P.oracle_gate_compact(gi, 1)
+    n_att = 10
+    cu = want["cu_seqlens"][:n_att + 1]
+    T = int(cu[-1])
+    q, k, v = wl.qkv(cfg, 2, T)
+    scale = wl.softmax_scale(cfg)
+    r = mosaic.stage_host(torch.from_numpy(gi.answers).pin_memory(),
+                          torch.from_numpy(gi.expert_conf).pin_memory(),
+                          torch.from_numpy(gi.ctx_len).pin_memory(), gi.tau, mosaic.CONF_WEIGHTED,
+                          q.pin_memory(), k.pin_memory(), v.pin_memory(), scale, max_attn_seqs=n_att)
+    S = int(r["n_survivors"])
+    assert S == want["n_survivors"] and int(r["total_tokens"]) == want["total_tokens"]
+    assert int(r["max_seqlen"]) == want["max_seqlen"]
+    assert np.array_equal(r["bypass"].numpy(), want["bypass"])
+    assert np.array_equal(r["mode"].numpy(), want["mode"])
+    assert np.array_equal(r["conf"].numpy().view(np.uint32), want["conf"].view(np.uint32))
+    assert np.array_equal(r["survivor_idx"][:S].numpy(), want["survivor_idx"])
+    assert np.array_equal(r["cu_seqlens"][:S + 1].numpy(), want["cu_seqlens"])
+    rs, rh, rp = wl.sample_rows(cu, cfg.Hq, cfg.Hkv, 2, cfg.config_id, n_random=128)
+    o = r["o"][:T]
+    lse = r["lse"][:cfg.Hq * T].view(cfg.Hq, T)
+    eo, el = P.check_attn_rows(o, lse, q, k, v, cu, rs, rh, rp, scale)
+    assert eo <= P.O_TOL and el <= P.LSE_TOL, (eo, el)
