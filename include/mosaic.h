@@ -391,7 +391,8 @@ mosaic_status_t mosaic_rope_packed(void* q, void* k, const int32_t* position_ids
  * inputs to the device, runs mosaic_gate_compact, reads S / total_tokens / max_seqlen back,
  * copies the survivors' packed Q/K/V to the device, runs mosaic_agg_prefill_attn and copies every
  * result back.  SYNCHRONOUS: returns after the results are in the host buffers.
- * The survivors' Q/K/V go up, through the attention kernel and back in chunks of whole sequences on
+ * The survivors' Q/K/V go up, through the attention kernel and back in chunks of ~8 k tokens (cut
+ * anywhere, also inside a sequence: a chunk's rows attend the keys uploaded so far) on
  * two internal copy streams (created on first use, one set per process), so the two PCIe
  * directions and the kernel overlap; concurrent calls from several threads serialise.
  *

@@ -1,18 +1,27 @@
 // stage.cu -- mosaic_stage_host: the whole confidence-gated aggregator stage (Alg. 1)
 // from HOST buffers: H2D copies, gate + compaction, survivors' prefill attention, D2H copies.
 // Only marshalling lives here; every step of the path runs in the kernels of gate.cu / attn.cu.
-// The survivors go through in chunks of whole sequences: chunk c+1 is on its way to the device
+// The survivors go through in chunks of ~8 k tokens (cut anywhere): chunk c+1 is on its way to the device
 // and the results of chunk c-1 on their way back while chunk c is in the attention kernel (PCIe
 // is full duplex, and at 2.6 GB per C2 step the copies are 94 % of the call).
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 #include <mutex>
+#include <vector>
 
 #include "common.cuh"
 
 namespace mosaic {
 namespace {
+
+#ifndef MOSAIC_STAGE_CHUNK_TOKENS
+#define MOSAIC_STAGE_CHUNK_TOKENS 8192
+#endif
+#ifndef MOSAIC_STAGE_MAX_CHUNKS
+#define MOSAIC_STAGE_MAX_CHUNKS 64
+#endif
+constexpr int kMaxChunks = MOSAIC_STAGE_MAX_CHUNKS;
 
 struct Arena {
     int32_t* answers;
@@ -32,6 +41,7 @@ struct Arena {
     float* lse;
     void* attn_ws;
     size_t attn_ws_bytes;
+    SeqDesc* views;  // one (q rows, key range) view per (chunk, sequence) overlap
     size_t total;
 };
 
@@ -67,19 +77,13 @@ Arena carve_arena(void* base, int64_t Q, int32_t E, int64_t T_cap, int32_t Hq, i
     const int64_t max_seqs = Q < T_cap ? Q : T_cap;
     a.attn_ws_bytes = mosaic_agg_prefill_attn_workspace_bytes((int32_t)max_seqs, T_cap, Hq, Hkv, D);
     a.attn_ws = take(a.attn_ws_bytes);
+    a.views = reinterpret_cast<SeqDesc*>(take((size_t)(max_seqs + kMaxChunks + 1) * sizeof(SeqDesc)));
     a.total = off;
     return a;
 }
 
 // Copy streams and events of the chunk pipeline (one set per process; the call is synchronous,
 // so one call uses them at a time -- concurrent calls serialise on the mutex).
-#ifndef MOSAIC_STAGE_CHUNK_TOKENS
-#define MOSAIC_STAGE_CHUNK_TOKENS 8192
-#endif
-#ifndef MOSAIC_STAGE_MAX_CHUNKS
-#define MOSAIC_STAGE_MAX_CHUNKS 16
-#endif
-constexpr int kMaxChunks = MOSAIC_STAGE_MAX_CHUNKS;
 struct Pipe {
     cudaStream_t in = nullptr, out = nullptr;
     cudaEvent_t ev_in[kMaxChunks], ev_out[kMaxChunks], ev_ready;
@@ -179,31 +183,47 @@ extern "C" mosaic_status_t mosaic_stage_host(
     if (T == 0) return MOSAIC_OK;
     if (T > T_cap) return MOSAIC_ERR_WORKSPACE_TOO_SMALL;
     if (!q_h || !k_h || !v_h || !o_h || !lse_h) return MOSAIC_ERR_INVALID_ARG;
-    // Chunks of whole sequences of about T / n_chunks tokens each (at least ~8 k tokens a chunk:
-    // smaller ones would make the attention launches and the copies latency-bound).
+    // Chunks of about T / n_chunks TOKENS each, cut anywhere -- also inside a sequence (at least
+    // ~8 k tokens a chunk: smaller ones would make the attention launches and the copies latency-
+    // bound).  The packed order is the upload order, so when chunk c has arrived every key its q
+    // rows may see has: the rows of sequence i inside the chunk, [r0, r1), attend that sequence's
+    // keys [0, r1) (bottom-right alignment, reading N2-1) -- one view per (chunk,
+    // sequence) overlap.  Cutting by tokens keeps the chunks equal (the first upload and the last
+    // attention + download are what the pipeline cannot hide) whatever the sequence lengths are.
     Pipe& pp = pipe();
     std::lock_guard<std::mutex> lock(pp.mu);
     if (!pipe_init(pp)) return MOSAIC_ERR_CUDA;
     int n_chunks = (int)(T / MOSAIC_STAGE_CHUNK_TOKENS);
     n_chunks = n_chunks < 1 ? 1 : (n_chunks > kMaxChunks ? kMaxChunks : n_chunks);
-    int64_t first[kMaxChunks + 1];  // first sequence of every chunk
+    std::vector<SeqDesc> views;
+    int first_view[kMaxChunks + 1];
+    int64_t bound[kMaxChunks + 1];
     {
-        int c = 0;
-        first[0] = 0;
-        for (int64_t q = 0; q < n_att && c + 1 < n_chunks; ++q)
-            if (cu_seqlens_h[q + 1] >= (T * (c + 1)) / n_chunks) first[++c] = q + 1;
-        n_chunks = c + 1;
-        first[n_chunks] = n_att;
+        int64_t seq = 0;
+        for (int c = 0; c <= n_chunks; ++c) bound[c] = T * c / n_chunks;
+        for (int c = 0; c < n_chunks; ++c) {
+            first_view[c] = (int)views.size();
+            const int64_t ta = bound[c], tb = bound[c + 1];
+            while (seq < n_att && cu_seqlens_h[seq + 1] <= ta) ++seq;
+            for (int64_t i = seq; i < n_att && cu_seqlens_h[i] < tb; ++i) {
+                const int64_t b0 = cu_seqlens_h[i], b1 = cu_seqlens_h[i + 1];
+                const int64_t r0 = ta > b0 ? ta : b0, r1 = tb < b1 ? tb : b1;
+                if (r1 > r0) views.push_back(SeqDesc{r0, b0, (int32_t)(r1 - r0), (int32_t)(r1 - b0)});
+            }
+        }
+        first_view[n_chunks] = (int)views.size();
     }
+    if (views.size() > (size_t)(n_att + kMaxChunks)) return MOSAIC_ERR_WORKSPACE_TOO_SMALL;
+    MOSAIC_CUDA_TRY(cudaMemcpyAsync(a.views, views.data(), views.size() * sizeof(SeqDesc), H2D, s));
     // the copy streams start after everything this call has enqueued on s so far
     MOSAIC_CUDA_TRY(cudaEventRecord(pp.ev_ready, s));
     MOSAIC_CUDA_TRY(cudaStreamWaitEvent(pp.in, pp.ev_ready, 0));
     MOSAIC_CUDA_TRY(cudaStreamWaitEvent(pp.out, pp.ev_ready, 0));
     const size_t q_row = (size_t)Hq * D * 2, kv_row = (size_t)Hkv * D * 2;
     for (int c = 0; c < n_chunks; ++c) {
-        const int64_t s0 = first[c], s1 = first[c + 1];
-        const int64_t t0 = cu_seqlens_h[s0], t1 = cu_seqlens_h[s1];
-        if (s1 == s0 || t1 == t0) continue;
+        const int64_t t0 = bound[c], t1 = bound[c + 1];
+        const int n_views = first_view[c + 1] - first_view[c];
+        if (t1 == t0 || n_views == 0) continue;
         const size_t rows = (size_t)(t1 - t0);
         auto at = [](const void* base, size_t off) { return static_cast<const char*>(base) + off; };
         auto at_w = [](void* base, size_t off) { return static_cast<char*>(base) + off; };
@@ -212,16 +232,14 @@ extern "C" mosaic_status_t mosaic_stage_host(
         MOSAIC_CUDA_TRY(cudaMemcpyAsync(at_w(a.v, t0 * kv_row), at(v_h, t0 * kv_row), rows * kv_row, H2D, pp.in));
         MOSAIC_CUDA_TRY(cudaEventRecord(pp.ev_in[c], pp.in));
         MOSAIC_CUDA_TRY(cudaStreamWaitEvent(s, pp.ev_in[c], 0));
-        // The sequences s0 .. s1-1 of the same packed buffers: cu_seqlens holds absolute offsets.
         // K and V are declared only as far as this chunk's last token (total_k_tokens = t1): the
         // last 128-row K / V box of the chunk reaches past it into rows whose copy (chunk c + 1)
         // may still be in flight -- those rows are masked, but a masked P = 0 times a stale NaN
         // pattern in V would still be NaN -- and rows past the tensor map's extent are zero-filled
         // by the TMA unit instead of being read.
-        st = mosaic_agg_prefill_attn_kv(a.q, a.k, a.v, a.cu_seqlens + s0, a.cu_seqlens + s0,
-                                        (int32_t)(s1 - s0), T, t1, sc.max_len, Hq, Hkv, D,
-                                        softmax_scale, /*causal=*/1, a.o, a.lse, a.attn_ws,
-                                        a.attn_ws_bytes, s);
+        st = attn_impl(a.q, a.k, a.v, nullptr, nullptr, a.views + first_view[c], n_views, T, t1,
+                       sc.max_len, Hq, Hkv, D, softmax_scale, /*causal=*/1, a.o, a.lse, a.attn_ws,
+                       a.attn_ws_bytes, s);
         if (st != MOSAIC_OK) {
             cudaStreamSynchronize(pp.in);
             cudaStreamSynchronize(s);
