@@ -99,51 +99,68 @@ extern "C" mosaic_status_t mosaic_lse_merge(const void* o_a, const float* lse_a,
 // ------------------------------------------------------------------------------------------
 // mosaic_lse_merge_n: the same merge for n partial results at once (the chunks of a split-KV
 // pass): LSE = ln sum_p e^LSE_p, O = sum_p O_p e^(LSE_p - LSE).  A thread takes 8 consecutive
-// elements of one (token, head) row and walks the n parts twice (the row's n logsumexps for the
-// maximum, then the weighted sum in fp32): every O_p element is read once.
+// elements of one (token, head) row and walks the n parts once, two at a time, with a running
+// maximum (an online softmax over the parts): every O_p element is read once.
 namespace mosaic {
 namespace {
-__global__ void __launch_bounds__(kMergeThreads) lse_merge_n_kernel(
+__device__ __forceinline__ float ex2_approx(float x) {  // 2^x, 2 ulp; 2^-inf = 0
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// What bounds this kernel is the bytes in flight per SM, i.e. occupancy: at 61 registers (four parts
+// in flight per thread, 4 blocks of 256 threads per SM) it ran at 5.0 TB/s; at 32 registers -- two
+// parts in flight, 16 blocks of 128 threads, all 2048 thread slots of an SM -- at 5.85 TB/s.
+// idx_t: 32-bit chunk / row indices whenever the call's chunk count fits (32-bit divisions).
+constexpr int kMergeNThreads = 128;
+constexpr int kMergeNBlocksPerSM = 16;
+constexpr int kMergeNInFlight = 2;  // parts in flight per thread
+template <typename idx_t>
+__global__ void __launch_bounds__(kMergeNThreads, kMergeNBlocksPerSM) lse_merge_n_kernel(
     const __nv_bfloat16* __restrict__ o_parts, const float* __restrict__ lse_parts, int n_parts,
     int64_t T, int Hq, int D, __nv_bfloat16* __restrict__ o, float* __restrict__ lse) {
-    const int per_row = D / 8;
-    const int64_t gid = (int64_t)blockIdx.x * kMergeThreads + threadIdx.x;
-    const int64_t rowi = gid / per_row;  // (token, head) row
-    if (rowi >= T * Hq) return;
-    const int c = (int)(gid - rowi * per_row);
-    const int64_t t = rowi / Hq;
-    const int h = (int)(rowi - t * Hq);
+    const idx_t per_row = (idx_t)(D / 8);
+    const idx_t gid = (idx_t)blockIdx.x * kMergeNThreads + threadIdx.x;  // 16-byte chunk of O
+    const idx_t rowi = gid / per_row;                                   // (token, head) row
+    if (rowi >= (idx_t)T * (idx_t)Hq) return;
+    const idx_t t = rowi / (idx_t)Hq;
+    const idx_t h = rowi - t * (idx_t)Hq;
     const int64_t o_stride = T * (int64_t)Hq * D, l_stride = (int64_t)Hq * T;
-    const float* lrow = lse_parts + (int64_t)h * T + t;
-    const __nv_bfloat16* orow = o_parts + rowi * D + c * 8;
-    // One pass, four parts in flight: running maximum m, weights relative to it, the accumulator
+    const float* lrow = lse_parts + (int64_t)h * T + (int64_t)t;
+    const __nv_bfloat16* orow = o_parts + (int64_t)gid * 8;
+    // One pass, PF parts in flight: running maximum m, weights relative to it, the accumulator
     // rescaled when the maximum moves (an empty partial -- LSE = -inf -- has weight 0 and its O,
     // which may be uninitialised, is multiplied by nothing).
+    constexpr float kLog2e = 1.4426950408889634f;
     float m = -INFINITY, z = 0.f;
     float acc[8];
 #pragma unroll
     for (int u = 0; u < 8; ++u) acc[u] = 0.f;
-    for (int p0 = 0; p0 < n_parts; p0 += 4) {
-        float l[4];
-        uint4 v[4];
+    constexpr int PF = kMergeNInFlight;
+    for (int p0 = 0; p0 < n_parts; p0 += PF) {
+        float l[PF];
+        uint4 v[PF];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
+        for (int j = 0; j < PF; ++j) {
             const bool in = p0 + j < n_parts;
             l[j] = in ? __ldg(lrow + (int64_t)(p0 + j) * l_stride) : -INFINITY;
             v[j] = in ? __ldcs(reinterpret_cast<const uint4*>(orow + (int64_t)(p0 + j) * o_stride))
                       : make_uint4(0u, 0u, 0u, 0u);
         }
-        const float m_new = fmaxf(fmaxf(m, fmaxf(l[0], l[1])), fmaxf(l[2], l[3]));
+        float m_new = m;
+#pragma unroll
+        for (int j = 0; j < PF; ++j) m_new = fmaxf(m_new, l[j]);
         if (m_new == -INFINITY) continue;
-        const float r = m == -INFINITY ? 0.f : expf(m - m_new);
+        const float r = ex2_approx((m - m_new) * kLog2e);  // m = -inf (nothing yet): 0
         z *= r;
 #pragma unroll
         for (int u = 0; u < 8; ++u) acc[u] *= r;
         m = m_new;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            if (l[j] == -INFINITY) continue;
-            const float w = expf(l[j] - m);
+        for (int j = 0; j < PF; ++j) {
+            const float w = ex2_approx((l[j] - m) * kLog2e);
+            if (w == 0.f) continue;
             z += w;
             const __nv_bfloat162* pv = reinterpret_cast<const __nv_bfloat162*>(&v[j]);
 #pragma unroll
@@ -159,8 +176,8 @@ __global__ void __launch_bounds__(kMergeThreads) lse_merge_n_kernel(
     __nv_bfloat162* po = reinterpret_cast<__nv_bfloat162*>(&out);
 #pragma unroll
     for (int u = 0; u < 4; ++u) po[u] = __floats2bfloat162_rn(acc[2 * u] * inv, acc[2 * u + 1] * inv);
-    *reinterpret_cast<uint4*>(o + rowi * D + c * 8) = out;
-    if (c == 0) lse[(int64_t)h * T + t] = z > 0.f ? m + logf(z) : -INFINITY;
+    *reinterpret_cast<uint4*>(o + (int64_t)gid * 8) = out;
+    if (gid == rowi * per_row) lse[(int64_t)h * T + (int64_t)t] = z > 0.f ? m + logf(z) : -INFINITY;
 }
 }  // namespace
 }  // namespace mosaic
@@ -174,11 +191,17 @@ extern "C" mosaic_status_t mosaic_lse_merge_n(const void* o_parts, const float* 
     if (!o_parts || !lse_parts || !o || !lse || !aligned16(o_parts) || !aligned16(o))
         return MOSAIC_ERR_INVALID_ARG;
     const int64_t threads = total_tokens * Hq * (D / 8);
-    const int64_t blocks = (threads + kMergeThreads - 1) / kMergeThreads;
+    const int64_t blocks = (threads + kMergeNThreads - 1) / kMergeNThreads;
     if (blocks >= (1ll << 31)) return MOSAIC_ERR_UNSUPPORTED;
-    lse_merge_n_kernel<<<(unsigned)blocks, kMergeThreads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
-        static_cast<const __nv_bfloat16*>(o_parts), lse_parts, n_parts, total_tokens, Hq, D,
-        static_cast<__nv_bfloat16*>(o), lse);
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    if (blocks * kMergeNThreads < (1ll << 32))
+        lse_merge_n_kernel<uint32_t><<<(unsigned)blocks, kMergeNThreads, 0, s>>>(
+            static_cast<const __nv_bfloat16*>(o_parts), lse_parts, n_parts, total_tokens, Hq, D,
+            static_cast<__nv_bfloat16*>(o), lse);
+    else
+        lse_merge_n_kernel<int64_t><<<(unsigned)blocks, kMergeNThreads, 0, s>>>(
+            static_cast<const __nv_bfloat16*>(o_parts), lse_parts, n_parts, total_tokens, Hq, D,
+            static_cast<__nv_bfloat16*>(o), lse);
     count_launch();
     MOSAIC_CUDA_TRY(cudaGetLastError());
     return MOSAIC_OK;
