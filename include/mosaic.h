@@ -356,6 +356,8 @@ mosaic_status_t mosaic_agg_decode_attn(const void* q, const void* k, const void*
  *   n_survivors, max_seqlen  host values read back from mosaic_compact.
  *   prompt_tokens [dev] int32, the prompts of all Q questions packed; prompt_off [dev] int64 [Q+1].
  *   trace_tokens  [dev] int32, the traces packed in (q, e) order; trace_off [dev] int64 [Q*E + 1].
+ *                 Both token buffers are read in whole 16-byte units (bulk copies): the 16-byte-
+ *                 aligned closure of each must be readable, which holds for any CUDA allocation.
  *   input_ids     [dev] int32 [total_tokens]  out: the packed contexts (16-byte aligned, as is
  *                 position_ids).
  *   position_ids  [dev] int32 [total_tokens]  out: 0, 1, ... inside every sequence.

@@ -5,18 +5,35 @@
 // (question q = survivor_idx[j]) is prompt(q) ++ trace(q, 0) ++ ... ++ trace(q, E-1).
 //
 // HBM-bound ragged gather: 4 bytes read and 8 written per token (token id, position id).  Block
-// (j, c) copies tokens [8192 c, 8192 c + 8192) of sequence j; a thread takes 4 consecutive tokens that
-// are 16-byte aligned in the output, so every full group is one 128-bit store per output array.
+// (j, c) copies tokens [8192 c, 8192 c + 8192) of sequence j.  The sources are 4-byte aligned runs of
+// any length, so they are fetched by bulk copies (TMA, `cp.async.bulk`) of the 16-byte-aligned
+// window around each run into a shared-memory ring -- the bytes in flight are the ring's, 32 KB
+// per block, where the first version (four 4-byte loads per thread and 16-byte stores: 4.7 TB/s)
+// was bound by the latency of what its registers could hold -- and written out lane-contiguous
+// from a 128-byte boundary of the output (whole-line stores, conflict-free shared-memory reads).
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 #include "common.cuh"
+#include "ptx.cuh"
 
 namespace mosaic {
 namespace {
 
 constexpr int kAsmThreads = 256;
-constexpr int kAsmChunk = 8192;  // tokens per block
+constexpr int kAsmChunk = 8192;   // tokens per block
+constexpr int kAsmPiece = 2048;   // tokens per bulk copy
+constexpr int kAsmStages = 4;     // bulk copies in flight per block (2-6 x 1-4 k tokens measure alike)
+constexpr int kAsmMaxPieces = kAsmChunk / kAsmPiece + MOSAIC_MAX_EXPERTS + 1;  // (a segment boundary ends a piece)
+
+struct AssembleSmem {
+    alignas(128) uint8_t stage[kAsmStages][kAsmPiece * 4 + 32];  // the aligned window of a piece
+    alignas(8) uint64_t full[kAsmStages];
+    int64_t piece_i[kAsmMaxPieces];           // first token (index in the sequence)
+    const int32_t* piece_src[kAsmMaxPieces];  // its address
+    int piece_n[kAsmMaxPieces];               // tokens
+    int n_pieces;
+};
 
 struct AssembleArgs {
     const int32_t* survivor_idx;
@@ -36,6 +53,15 @@ __global__ void __launch_bounds__(kAsmThreads) assemble_kernel(const AssembleArg
     // address of segment g's first token minus cum[g], so token i of the sequence is src[g][i].
     __shared__ int64_t cum[MOSAIC_MAX_EXPERTS + 2];
     __shared__ const int32_t* src[MOSAIC_MAX_EXPERTS + 1];
+    __shared__ AssembleSmem sm;
+    auto fetch = [&](int q) {  // piece q -> its stage of the ring
+        const uintptr_t a = reinterpret_cast<uintptr_t>(sm.piece_src[q]);
+        const uintptr_t lo = a & ~uintptr_t(15), hi = (a + 4u * (uintptr_t)sm.piece_n[q] + 15u) & ~uintptr_t(15);
+        const uint32_t bar = ptx::smem_u32(&sm.full[q % kAsmStages]);
+        ptx::mbar_arrive_expect_tx(bar, (uint32_t)(hi - lo));
+        ptx::bulk_load_1d(ptx::smem_u32(sm.stage[q % kAsmStages]), reinterpret_cast<const void*>(lo),
+                          (uint32_t)(hi - lo), bar);
+    };
     const int j = blockIdx.x;
     const int64_t t0 = p.cu_seqlens[j];
     const int64_t L = p.cu_seqlens[j + 1] - t0;
@@ -80,51 +106,55 @@ __global__ void __launch_bounds__(kAsmThreads) assemble_kernel(const AssembleArg
     __syncthreads();
     const int64_t i1 = min(L, i0 + kAsmChunk);
     const int64_t total = cum[nseg];
-    auto token = [&](int64_t i) -> int32_t {
-        if (i >= total) return -1;  // past the sources of a sequence whose length does not match them
-        int g = 0;
-        for (int k = 1; k < nseg; ++k) g += (i >= cum[k]) ? 1 : 0;  // (empty segments are skipped)
-        return __ldg(src[g] + i);
-    };
-    // Groups of 4 tokens aligned to 16 bytes in the OUTPUT arrays (the sequence starts anywhere):
-    // group k of this block covers output elements [base + 4 k, base + 4 k + 4); a full group is one
-    // 16-byte store per array, the ragged first and last groups are written element by element.
-    // (Staging the tokens through shared memory for fully coalesced loads was measured slower:
-    //  153 against 132 us on the bench workload.)
-    const int64_t base = (t0 + i0) & ~int64_t(3);
-    const int64_t n_groups = (t0 + i1 - base + 3) >> 2;
-#pragma unroll 2
-    for (int64_t k = threadIdx.x; k < n_groups; k += kAsmThreads) {
-        const int64_t o = base + 4 * k;  // output element of the group's first token
-        const int64_t i = o - t0;        // its index in the sequence (may be < i0 in the first group)
-        if (i >= i0 && i + 4 <= i1) {
-            int4 tk, ps;
-            int g = 0;
-            for (int kk = 1; kk < nseg; ++kk) g += (i >= cum[kk]) ? 1 : 0;
-            if (i + 4 <= cum[g + 1]) {  // the usual case: all four in one segment, one search
-                const int32_t* from = src[g] + i;
-                tk.x = __ldg(from);
-                tk.y = __ldg(from + 1);
-                tk.z = __ldg(from + 2);
-                tk.w = __ldg(from + 3);
-            } else {
-                tk.x = token(i);
-                tk.y = token(i + 1);
-                tk.z = token(i + 2);
-                tk.w = token(i + 3);
-            }
-            ps = make_int4((int)i, (int)i + 1, (int)i + 2, (int)i + 3);
-            __stcs(reinterpret_cast<int4*>(p.input_ids + o), tk);
-            __stcs(reinterpret_cast<int4*>(p.position_ids + o), ps);
-        } else {
-            for (int u = 0; u < 4; ++u) {
-                const int64_t iu = i + u;
-                if (iu >= i0 && iu < i1) {
-                    __stcs(p.input_ids + o + u, token(iu));
-                    __stcs(p.position_ids + o + u, (int32_t)iu);
-                }
+    const int64_t have = min(i1, total);  // tokens of the chunk that have a source: [i0, have)
+    // The chunk's tokens come from PIECES: runs of at most kAsmPiece tokens inside one segment.
+    // Thread 0 lists them and fetches each with one bulk copy (the 16-byte-aligned window around
+    // the run: sources are 4-byte aligned) into a ring of kAsmStages buffers; all threads then move
+    // a piece from shared memory to the two outputs.  The bytes in flight are the ring's, not the
+    // registers': kAsmStages x 8 KB per block.
+    if (threadIdx.x == 0) {
+        int np = 0, g = 0;
+        for (int64_t pos = i0; pos < have;) {
+            while (cum[g + 1] <= pos) ++g;  // (empty segments are skipped)
+            const int64_t n = min(min(have, cum[g + 1]), pos + kAsmPiece) - pos;
+            sm.piece_i[np] = pos;
+            sm.piece_n[np] = (int)n;
+            sm.piece_src[np] = src[g] + pos;
+            ++np;
+            pos += n;
+        }
+        sm.n_pieces = np;
+        for (int s = 0; s < kAsmStages; ++s) ptx::mbar_init(ptx::smem_u32(&sm.full[s]), 1);
+        ptx::fence_barrier_init();
+        for (int q = 0; q < np && q < kAsmStages; ++q) fetch(q);
+    }
+    __syncthreads();
+    const int np = sm.n_pieces;
+    for (int q = 0; q < np; ++q) {
+        const int s = q % kAsmStages;
+        ptx::mbar_wait(ptx::smem_u32(&sm.full[s]), (uint32_t)(q / kAsmStages) & 1u);
+        const int64_t pi = sm.piece_i[q];
+        const int n = sm.piece_n[q];
+        const int32_t* st = reinterpret_cast<const int32_t*>(sm.stage[s]) +
+                            ((reinterpret_cast<uintptr_t>(sm.piece_src[q]) & 15u) >> 2);
+        // lane-contiguous, starting at a 128-byte boundary of the OUTPUT: a warp's stores are whole
+        // lines, its shared-memory reads conflict-free
+        const int64_t o0 = t0 + pi;
+        const int first = (int)((o0 & ~int64_t(31)) - o0) + (int)threadIdx.x;  // may be < 0
+#pragma unroll 4
+        for (int k = first; k < n; k += kAsmThreads) {
+            if (k >= 0) {
+                __stcs(p.input_ids + o0 + k, st[k]);
+                __stcs(p.position_ids + o0 + k, (int32_t)(pi + k));
             }
         }
+        __syncthreads();  // the stage is free
+        if (threadIdx.x == 0 && q + kAsmStages < np) fetch(q + kAsmStages);
+    }
+    // past the sources of a sequence whose length does not match them
+    for (int64_t i = max(i0, total) + threadIdx.x; i < i1; i += kAsmThreads) {
+        __stcs(p.input_ids + t0 + i, -1);
+        __stcs(p.position_ids + t0 + i, (int32_t)i);
     }
 }
 
