@@ -447,7 +447,8 @@ def bench_lse_merge_n(torch, mosaic, pk, T, Hq, D, n=4):
     o = torch.empty((T, Hq, D), dtype=torch.bfloat16, device=dev)
     lse = torch.empty((Hq, T), dtype=torch.float32, device=dev)
     ms = timed(torch, lambda: mosaic.lse_merge_n(op, lp, o=o, lse=lse), 20)   # 5.7 GB: cold
-    return hbm_leg(ms, 2.0 * (n + 1) * T * Hq * D + 4.0 * (n + 1) * T * Hq, pk)
+    return hbm_leg(ms, 2.0 * (n + 1) * T * Hq * D + 4.0 * (n + 1) * T * Hq, pk,
+                   static_traffic("lse_merge_n_dram_bytes_per_launch"))
 
 
 def bench_prefix(torch, mosaic, pk):
