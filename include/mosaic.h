@@ -119,6 +119,26 @@ mosaic_status_t mosaic_compact(const uint8_t* bypass, const int32_t* ctx_len, in
                                size_t workspace_bytes, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * mosaic_compact_static -- mosaic_compact (Alg. 1 line 6; same arguments, same results
+ * bit for bit) WITHOUT a caller workspace, for callers that cannot allocate device memory (code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  The scan
+ * state lives in a 1 MiB device array inside the library, which every GPU that loads the library
+ * holds until the process exits; the call allocates nothing (no cudaMalloc / cudaFree / allocating
+ * library routine) and zeroes the part of the array it uses on the stream before it scans.
+ *
+ *   Q > MOSAIC_COMPACT_STATIC_MAX_Q returns MOSAIC_ERR_WORKSPACE_TOO_SMALL (the array holds the
+ *   scan state of at most that many questions); use mosaic_compact with a workspace there.
+ *   Every call on a device shares the one array: calls that overlap on the GPU (different
+ *   streams, several host threads) RACE and give undefined results -- keep them on one stream or
+ *   order them with events.  Calls on different devices are independent.
+ * ------------------------------------------------------------------------------------------- */
+#define MOSAIC_COMPACT_STATIC_MAX_Q (1 << 22)
+mosaic_status_t mosaic_compact_static(const uint8_t* bypass, const int32_t* ctx_len, int64_t Q,
+                                      int32_t* survivor_idx, int64_t* cu_seqlens,
+                                      int32_t* n_survivors, int64_t* total_tokens,
+                                      int32_t* max_seqlen, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * mosaic_gate_compact -- mosaic_gate followed by mosaic_compact in ONE kernel launch (the
  * bypass mask never makes a round trip through HBM before the scan), async.  Same arguments,
  * same results bit for bit; bypass_out may be NULL here.  Workspace: mosaic_compact's.

@@ -14,7 +14,7 @@ CSRC = PKG / "csrc"
 INCLUDE = ROOT / "include"
 LIB = PKG / "libmosaic.so"
 OBJ_DIR = PKG / "build"
-SOURCES = ["core.cu", "gate.cu", "compact.cu", "compact_inst_c0a0.cu", "compact_inst_c0a1.cu",
+SOURCES = ["core.cu", "gate.cu", "compact.cu", "compact_static.cu", "compact_inst_c0a0.cu", "compact_inst_c0a1.cu",
            "compact_inst_c1a0.cu", "compact_inst_c1a1.cu", "compact_inst_c2a0.cu",
            "compact_inst_c2a1.cu", "attn.cu", "stage.cu", "assemble.cu", "rope.cu", "merge.cu", "decode.cu", "cascade.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -26,6 +26,7 @@ SIGNATURES = {
     "mosaic_gate": (ctypes.c_int, [_vp, _vp, _i64, _i32, _f32, _i32, _vp, _vp, _vp, _vp, _vp, _vp]),
     "mosaic_compact_workspace_bytes": (_sz, [_i64]),
     "mosaic_compact": (ctypes.c_int, [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "mosaic_compact_static": (ctypes.c_int, [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp]),
     "mosaic_gate_compact": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _f32, _i32, _vp, _vp, _vp,
                                            _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     "mosaic_gate_compact_tau": (ctypes.c_int, [_vp, _vp, _vp, _i64, _i32, _vp, _i32, _vp, _vp, _vp,
@@ -170,6 +171,26 @@ def compact(bypass, ctx_len, *, out=None, stream=None):
                                r["workspace"].numel(), _stream(stream))
     _check("mosaic_compact", st)
     return r
+
+
+COMPACT_STATIC_MAX_Q = 1 << 22
+
+
+def compact_static(bypass, ctx_len, *, out, stream=None):
+    """mosaic_compact_static: mosaic_compact with the scan state in the library's own device array.
+    The call allocates nothing, so neither does this wrapper: `out` must hold survivor_idx [Q]
+    int32, cu_seqlens [Q+1] int64 and the device scalars n_survivors, total_tokens, max_seqlen."""
+    Q = bypass.shape[0]
+    st = load().mosaic_compact_static(_dptr(bypass, torch.uint8, "bypass"),
+                                      _dptr(ctx_len, torch.int32, "ctx_len"), Q,
+                                      _dptr(out["survivor_idx"], torch.int32, "survivor_idx"),
+                                      _dptr(out["cu_seqlens"], torch.int64, "cu_seqlens"),
+                                      _dptr(out["n_survivors"], torch.int32, "n_survivors"),
+                                      _dptr(out["total_tokens"], torch.int64, "total_tokens"),
+                                      _dptr(out["max_seqlen"], torch.int32, "max_seqlen"),
+                                      _stream(stream))
+    _check("mosaic_compact_static", st)
+    return out
 
 
 def gate_compact(answers, ctx_len, tau, expert_conf=None, conf_mode=CONF_VOTE, *, want_count=False,
