@@ -813,10 +813,22 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                 for (int c = 0; c < BS / 32; ++c)
                     ptx::tmem_ld32(tSb + c * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[c * 32]));
                 ptx::tmem_wait_ld();
+                // kMask 1: thr does not decrease with the lane; when even the warp's last row sees
+                // none of the step's second 32 keys their exponentials are skipped (P = 0)
+                bool skip1 = false;
                 if constexpr (kMask == 1) {
+                    skip1 = __shfl_sync(0xffffffffu, thr, 31) < 32;
+                    const int thr_lo = __shfl_sync(0xffffffffu, thr, 0);
+                    if (thr_lo < 31) {  // (else every row of the warp sees the first 32 keys)
 #pragma unroll
-                    for (int c = 0; c < BS; ++c)
-                        if (c > thr) s[c] = -INFINITY;
+                        for (int c = 0; c < 32; ++c)
+                            if (c > thr) s[c] = -INFINITY;
+                    }
+                    if (thr_lo < 63) {
+#pragma unroll
+                        for (int c = 32; c < BS; ++c)
+                            if (c > thr) s[c] = -INFINITY;
+                    }
                 }
                 float mx0 = s[0], mx1 = s[1], mx2 = s[2], mx3 = s[3];
 #pragma unroll
@@ -829,7 +841,9 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
                 const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
                 const float m_new = mx * sc;
                 if (first) {
-                    m_used = m_new;
+                    // (a row that sees no key at all -- only against the contract, Lk < Lq -- keeps
+                    //  a finite max, so that its masked scores give exp2(-inf) = 0, not NaN)
+                    m_used = kMask == 1 ? fmaxf(m_new, -1e30f) : m_new;
                 } else {
                     // move the max (and rescale l, O) only when it grew by more than 2^8
                     const bool need = m_new > m_used + kRescaleThreshold;
@@ -872,16 +886,19 @@ attn_fwd(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUten
 #pragma unroll
                 for (int c = 0; c < BS / 32; ++c) {
                     uint32_t pk[16];
+                    if (kMask == 1 && c == 1 && skip1) {  // no row of the warp sees these 32 keys
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) pk[i] = 0u;
+                        ptx::tmem_st16(tSb + c * 16, pk);
+                        continue;
+                    }
 #pragma unroll
                     for (int i = 0; i < 32; i += 2) {
                         const float x0 = s[c * 32 + i], x1 = s[c * 32 + i + 1];
                         float2 e;
-                        if constexpr (kMask == 1) {
-                            // a masked key must give exactly 0 even when scale_log2 == 0 (-inf * 0)
-                            const float a0 = fmaf(x0, sc, -m_used), a1 = fmaf(x1, sc, -m_used);
-                            e.x = ex2_approx(x0 == -INFINITY ? -INFINITY : a0);
-                            e.y = ex2_approx(x1 == -INFINITY ? -INFINITY : a1);
-                        } else {
+                        {
+                            // (a masked key is -inf and scale_log2 > 0 -- the host keeps it above
+                            //  2^-100 even for softmax_scale = 0 -- so it gives exp2(-inf) = 0)
                             const float2 a = __ffma2_rn(make_float2(x0, x1), sc2, nm2);
                             if (((i >> 1) & 3) < kPolyPairs)
                                 e = exp2_poly2(a);
@@ -1088,7 +1105,9 @@ mosaic_status_t attn_impl(const void* q, const void* k, const void* v, const int
     p.T = total_tokens;
     p.Hq = Hq;
     p.Hkv = Hkv;
-    p.scale_log2 = fabsf(softmax_scale) * kLog2e;
+    // (kept positive: a masked score is -inf and must stay -inf under the scale -- 0 x -inf is NaN;
+    //  at 2^-100 every real score still scales to 0 to all fp32 digits, i.e. softmax_scale = 0)
+    p.scale_log2 = fmaxf(fabsf(softmax_scale) * kLog2e, 7.8886091e-31f);
     p.inv_group = 1.0f / (float)(Hq / Hkv);
     p.group = Hq / Hkv;
     p.causal = causal ? 1 : 0;
