@@ -6,6 +6,8 @@ import pytest
 import torch
 
 import _parity as P
+import oracle
+from paper_2606_03014_b200 import mosaic
 from paper_2606_03014_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
@@ -123,3 +125,35 @@ def test_n4_paper_shaped_workload_bit_exact(seed):
             P.assert_gate_equal(fused, want)
         assert 0.80 < 1.0 - P.oracle_gate_compact(wl.GateInputs(a, None, ctx, 2.0 / 3.0, 3), 0)[
             "n_survivors"] / Q < 0.89   # Table 1: 84.62 % skipped at tau = 2/3
+
+
+def _wide_weights(g, Q, E):
+    """fp32 weights spread over 2^+-40 with zeros and all-zero rows: the binary64 sums round (a
+    kernel that accumulated in fp32, or dropped the small terms, would show in conf's bits)."""
+    w = np.exp2(g.uniform(-40.0, 40.0, size=(Q, E))).astype(np.float32)
+    w[g.random((Q, E)) < 0.1] = 0.0
+    w[::97] = 0.0                                            # St = 0: conf falls back to agree
+    return w
+
+
+@pytest.mark.parametrize("E", [3, 5, 8, 13])
+def test_weights_of_very_different_magnitudes(E):
+    g = np.random.default_rng(500 + E)
+    Q = 30011
+    a = g.integers(0, 3, size=(Q, E), dtype=np.int32)
+    w = _wide_weights(g, Q, E)
+    ctx = g.integers(0, 50000, size=Q, dtype=np.int32)
+    gi = wl.GateInputs(a, w, ctx, 0.6, E)
+    want = P.oracle_gate_compact(gi, 1)
+    assert 0.05 < want["bypass"].mean() < 0.95              # both outcomes occur
+    sep, fused = P.gpu_gate_compact_all(gi, 1)
+    P.assert_gate_equal(sep, want)
+    P.assert_gate_equal(fused, want)
+    # the weighted-argmax estimator: per-label sums, ties between labels included (zero rows)
+    want2 = oracle.gate_ext(a, 0.6, w, 2)
+    r = mosaic.gate_compact_ext(torch.from_numpy(a).cuda(), torch.from_numpy(ctx).cuda(), 0.6,
+                                torch.from_numpy(w).cuda(), 2)
+    torch.cuda.synchronize()
+    assert np.array_equal(r["mode"].cpu().numpy(), want2["mode"])
+    assert np.array_equal(r["conf"].cpu().numpy().view(np.uint32), want2["conf"].view(np.uint32))
+    assert np.array_equal(r["bypass"].cpu().numpy(), want2["bypass"])
