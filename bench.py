@@ -321,7 +321,25 @@ def bench_gate_c5(torch, mosaic, wl, pk, gi, steps=80, warmup=8):
     ms = timed(torch, graph.replay, max(3, steps // nsets), max(1, warmup // nsets)) / nsets
     t = float(np.median(ms)) * 1e-3
     gbs = byts / t / 1e9
+    # Context for a 90 MB call (Kernel G): the simplest kernel there is -- torch's
+    # elementwise fp32 copy -- moving the same number of bytes in the same harness.  Not ours, not
+    # counted in gpu_launches; it says what fraction of the copy bandwidth ANY kernel reaches here.
+    n = int(byts) // 8 // 1024 * 1024
+    cp = [(torch.empty(n, dtype=torch.float32, device="cuda").normal_(),
+           torch.empty(n, dtype=torch.float32, device="cuda")) for _ in range(nsets)]
+    with torch.cuda.stream(side):
+        for x, y in cp:
+            torch.mul(x, 1.0, out=y)
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    cgraph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(cgraph):
+        for x, y in cp:
+            torch.mul(x, 1.0, out=y)
+    cms = timed(torch, cgraph.replay, max(3, steps // nsets), max(1, warmup // nsets)) / nsets
+    copy_us = float(np.median(cms)) * 1e3
     return {"workload": "configs[4]: Q=2^20, E=8, weighted conf, p=0.6, tau=0.75",
+            "copy_same_bytes_us": r3(copy_us),
             "mqueries_per_s": r3(cfg.Q / t / 1e6), "us_per_call": r3(t * 1e6),
             "us_best": r3(float(ms.min()) * 1e3), "survivors": S,
             "kernels_per_call": int(launches_per_call),
