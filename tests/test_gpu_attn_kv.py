@@ -132,3 +132,33 @@ def test_merge_against_the_oracle_and_empty_partials():
     fin = np.isfinite(l_ref)
     assert np.array_equal(np.isneginf(lg), np.isneginf(l_ref))
     assert np.abs(lg[fin] - l_ref[fin]).max() <= 1e-5 * (1 + np.abs(l_ref[fin]).max())
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2, 3, 4, 5])
+def test_random_shapes(seed):
+    """Seeded random batches: q lengths 0..400, 0..900 more keys than q rows, both head sizes, three
+    group sizes, causal and not -- every row against the oracle."""
+    g = np.random.default_rng(900 + seed)
+    Hq, Hkv = [(4, 2), (6, 1), (8, 8)][seed % 3]
+    D = (128, 64)[seed % 2]
+    causal = seed % 4 != 3
+    n = 14
+    Lq = g.integers(0, 401, size=n)
+    Lq[g.integers(0, n)] = 0                                   # an empty q sequence somewhere
+    Lk = Lq + g.integers(0, 901, size=n) * (g.random(n) < 0.7)  # 30 % plain sequences
+    Lk = np.maximum(Lk, 1)                                      # (a q row needs a key)
+    cq, ck = _cu(Lq), _cu(Lk)
+    q = P.randn_bf16((int(cq[-1]), Hq, D), 7 * seed)
+    k = P.randn_bf16((int(ck[-1]), Hkv, D), 7 * seed + 1, 1.5)
+    v = P.randn_bf16((int(ck[-1]), Hkv, D), 7 * seed + 2)
+    scale = 1.0 / np.sqrt(D)
+    o, lse = mosaic.agg_prefill_attn_kv(q.cuda(), k.cuda(), v.cuda(), torch.from_numpy(cq).cuda(),
+                                        torch.from_numpy(ck).cuda(), n, int(Lq.max()), scale,
+                                        causal=causal)
+    torch.cuda.synchronize()
+    O_ref, lse_ref = oracle.attn_kv_full(P.bf16_bits(q), P.bf16_bits(k), P.bf16_bits(v), cq, ck, scale,
+                                         causal=causal)
+    assert np.all(np.isfinite(lse.cpu().numpy()))
+    eo = float(np.abs(o.float().cpu().numpy() - O_ref).max())
+    el = float(np.abs(lse.cpu().numpy() - lse_ref).max())
+    assert eo <= P.O_TOL and el <= P.LSE_TOL, (seed, eo, el)
