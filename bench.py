@@ -47,7 +47,7 @@ def peaks():
     if p.exists():
         d = json.loads(p.read_text())
         d.setdefault("bf16_tflops_sustained", d["bf16_tflops"])
-        return d, "measured (MEASURED_PEAKS.json)"
+        return d, "MEASURED_PEAKS.json"
     return dict(FALLBACK_PEAKS), "fallback (B200_PROFILING.md)"
 
 
@@ -213,9 +213,9 @@ def oracle_sample(cfg, seed, budget_rows):
 
 
 def workload_name(cfg):
-    return (f"{cfg.name} (BASELINE.json configs[{cfg.config_id - 1}]): gate+compaction over "
-            f"2^20 questions (E=8, weighted conf), attention over the first {cfg.max_attn_seqs} "
-            f"survivors (Hq/Hkv/D={cfg.Hq}/{cfg.Hkv}/{cfg.D}, 8-32 k tokens)")
+    return (f"{cfg.name} (configs[{cfg.config_id - 1}]): gate+compaction of 2^20 questions "
+            f"(E=8, weighted) + attention of the first {cfg.max_attn_seqs} survivors "
+            f"({cfg.Hq}/{cfg.Hkv}/{cfg.D}, 8-32 k tokens)")
 
 
 def run_reference(args):
@@ -790,7 +790,7 @@ def run_product(args):
         "config": {"workload": workload_name(cfg), "Q": cfg.Q, "E": cfg.E, "tau": cfg.tau,
                    "survivors": S_all, "attn_seqs": S, "total_tokens": T, "max_seqlen": max_len,
                    "per_rank_seed": "rank", "tflop_per_step": r3(flops / 1e12),
-                   "l2": "inputs larger than L2 (Q+K+V+O = %.1f GB per step)" %
+                   "l2": "inputs > L2 (Q+K+V+O = %.1f GB per step)" %
                          ((2 * T * cfg.Hq + 2 * T * cfg.Hkv) * cfg.D * 2 / 1e9),
                    "gate_ms_in_step": r3(float(np.median(gate_ms))), "peaks": pk_src},
         "roofline": {"bound": "tensor", "achieved": r3(attn_tflops), "peak": peak,
