@@ -157,3 +157,26 @@ def test_weights_of_very_different_magnitudes(E):
     assert np.array_equal(r["mode"].cpu().numpy(), want2["mode"])
     assert np.array_equal(r["conf"].cpu().numpy().view(np.uint32), want2["conf"].view(np.uint32))
     assert np.array_equal(r["bypass"].cpu().numpy(), want2["bypass"])
+
+
+def test_sixteen_million_questions_bit_exact():
+    """2^24 + 12 345 questions (E = 8, weighted): ~57 tiles per block of the persistent grid, a ragged
+    last tile, token totals far beyond 2^31 -- the size of bench.py's supplementary gate point."""
+    cfg = wl.C5
+    Q = (1 << 24) + 12345
+    gi = wl.gate_inputs(cfg, 3, Q=Q)
+    want = P.oracle_gate_compact(gi, 1)
+    assert want["total_tokens"] > 2 ** 37
+    a = torch.from_numpy(gi.answers).cuda()
+    w = torch.from_numpy(gi.expert_conf).cuda()
+    cl = torch.from_numpy(gi.ctx_len).cuda()
+    for _ in range(2):                                        # (the second call reuses the workspace)
+        r = mosaic.gate_compact(a, cl, gi.tau, w, 1, want_count=True, want_agree=True)
+        torch.cuda.synchronize()
+        S = int(r["n_survivors"])
+        got = dict(mode=r["mode"].cpu().numpy(), count=r["count"].cpu().numpy(),
+                   agree=r["agree"].cpu().numpy(), conf=r["conf"].cpu().numpy(),
+                   bypass=r["bypass"].cpu().numpy(), survivor_idx=r["survivor_idx"][:S].cpu().numpy(),
+                   cu_seqlens=r["cu_seqlens"][:S + 1].cpu().numpy(), n_survivors=S,
+                   total_tokens=int(r["total_tokens"]), max_seqlen=int(r["max_seqlen"]))
+        P.assert_gate_equal(got, want)
