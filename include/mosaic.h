@@ -131,6 +131,8 @@ mosaic_status_t mosaic_compact(const uint8_t* bypass, const int32_t* ctx_len, in
  *   Every call on a device shares the one array: calls that overlap on the GPU (different
  *   streams, several host threads) RACE and give undefined results -- keep them on one stream or
  *   order them with events.  Calls on different devices are independent.
+ *   The first call on a device asks the runtime for the array's address (cudaGetSymbolAddress, which
+ *   may load the module): make that call outside a stream capture; later calls only launch kernels.
  * ------------------------------------------------------------------------------------------- */
 #define MOSAIC_COMPACT_STATIC_MAX_Q (1 << 22)
 mosaic_status_t mosaic_compact_static(const uint8_t* bypass, const int32_t* ctx_len, int64_t Q,
