@@ -109,3 +109,30 @@ def test_maximum_size_and_beyond():
     assert e.value.status == mosaic.ERR_WORKSPACE_TOO_SMALL
     torch.cuda.synchronize()
     assert int(out["n_survivors"]) == -5
+
+
+def test_replays_inside_a_cuda_graph():
+    """What the entry point is for: after one ordinary call (which asks for the array's address), the
+    call is captured into a CUDA graph -- where allocating is not allowed -- and replayed."""
+    Q = 300_000
+    bypass, ctx_len = _inputs(Q, 0.6, 6)
+    b, c = torch.from_numpy(bypass).cuda(), torch.from_numpy(ctx_len).cuda()
+    out = _outputs(Q, -1)
+    mosaic.compact_static(b, c, out=out)                       # warm-up, outside the capture
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            mosaic.compact_static(b, c, out=out, stream=side)
+    torch.cuda.current_stream().wait_stream(side)
+    ref = mosaic.compact(b, c)
+    torch.cuda.synchronize()
+    S = int(ref["n_survivors"])
+    for _ in range(2):
+        for t in out.values():
+            t.fill_(-1)
+        graph.replay()
+        torch.cuda.synchronize()
+        _same(out, ref, S)
